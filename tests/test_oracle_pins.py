@@ -1,0 +1,335 @@
+"""Pins of the CPU oracle against things other than itself (prompt section (3)).
+
+Every test here fails for a plausible mistake in oracle/sg_oracle.c: a dropped term, a wrong sign,
+a swapped corner, x/y transposed, a wrong coincidence rule.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import oracle
+from workloads import (Layout, cell_rects, make_config, paper_ilr_layout, paper_vlr_layout,
+                       d2_sigma, d2_slopes, d22_sigma, d22_slopes, nested_layout, kuzmin_sigma)
+from workloads.configs import uniform_layout, cell_centres, _sorted_patches
+
+
+# ------------------------------------------------------------------------------------------
+# helpers that do NOT restate the oracle's closed forms: brute-force quadrature and analytic disks
+# ------------------------------------------------------------------------------------------
+def quad_kernels(xl, xr, yd, yu, x, y):
+    """The six kernel integrals of PAPER.md:90 by adaptive 2-D quadrature (target outside the cell)."""
+    xc, yc = 0.5 * (xl + xr), 0.5 * (yd + yu)
+
+    def q(f):
+        return integrate.dblquad(lambda yb, xb: f(xb - x, yb - y, xb, yb), xl, xr, yd, yu,
+                                 epsabs=1e-13, epsrel=1e-12)[0]
+
+    r3 = lambda u, v: (u * u + v * v) ** 1.5
+    return np.array([
+        q(lambda u, v, xb, yb: u / r3(u, v)),
+        q(lambda u, v, xb, yb: (xb - xc) * u / r3(u, v)),
+        q(lambda u, v, xb, yb: (yb - yc) * u / r3(u, v)),
+        q(lambda u, v, xb, yb: v / r3(u, v)),
+        q(lambda u, v, xb, yb: (xb - xc) * v / r3(u, v)),
+        q(lambda u, v, xb, yb: (yb - yc) * v / r3(u, v)),
+    ])
+
+
+def FR_D2(R, a=0.5):
+    """PAPER.md:132 Eq. 9 (second branch is R > alpha; sigma0 = G = 1)."""
+    R = np.asarray(R, float)
+    out = np.empty_like(R)
+    i = R <= a
+    out[i] = -(3 * np.pi ** 2 * R[i] / (16 * a ** 3)) * (4 * a * a - 3 * R[i] ** 2)
+    Ro = R[~i]
+    out[~i] = -(3 * np.pi / (8 * a ** 3)) * (Ro * (4 * a * a - 3 * Ro ** 2) * np.arcsin(a / Ro)
+                                             - a * (2 * a * a - 3 * Ro ** 2) * np.sqrt(1 - a * a / Ro ** 2))
+    return out
+
+
+def F_D2_xy(x, y, a, xc=0.0, yc=0.0):
+    R = np.hypot(x - xc, y - yc)
+    fr = FR_D2(R, a)
+    return fr * (x - xc) / R, fr * (y - yc) / R
+
+
+def fig1_layout():
+    """Fig. 1 / Table 10 example rebuilt from its description: 4x4 zones on [0,1]^2,
+    zones 6 and 11 refined, then zone 17 (upper-left child of 6) and 19 (lower-right child of 6)."""
+    l0 = [(0, i, j) for j in range(4) for i in range(4) if (i, j) not in ((1, 1), (2, 2))]
+    l1 = [(1, 2, 2), (1, 3, 3)]                                   # zones 18 (LL of 6), 20 (UR of 6)
+    l1 += [(1, 4 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]  # zones 21-24 (children of 11)
+    l2 = [(2, 4 + di, 6 + dj) for dj in (0, 1) for di in (0, 1)]   # children of 17 = cell (2,3) of level 1
+    l2 += [(2, 6 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]  # children of 19 = cell (3,2) of level 1
+    return Layout(3, np.array([0.25, 0.125, 0.0625]), 0.0, 0.0, 1, _sorted_patches(l0 + l1 + l2))
+
+
+# ------------------------------------------------------------------------------------------
+# P0: closed forms vs quadrature
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("rect,tgt", [
+    ((64, 96, 16, 48), (19, -13)),       # generic, target left/below
+    ((-40, -8, 10, 20), (33, 47)),       # target right/above: every corner has v < 0 and u < 0
+    ((-12, 20, 30, 50), (5, 3)),         # target below the cell, inside its x-range (u changes sign)
+    ((10, 30, -40, 8), (-7, -2)),        # target left of the cell, inside its y-range (v changes sign)
+])
+def test_P0_six_kernels_vs_quadrature(rect, tgt):
+    unit = 1 / 64
+    K = oracle.cell_kernels(*rect, *tgt, unit)
+    Q = quad_kernels(*(np.array(rect) * unit), tgt[0] * unit, tgt[1] * unit)
+    np.testing.assert_allclose(K, Q, rtol=0, atol=2e-11)
+
+
+@pytest.mark.parametrize("rect,tgt", [
+    ((8, 24, 4, 20), (8, -6)),      # u == 0 on the left edge, target below
+    ((8, 24, 4, 20), (24, 31)),     # u == 0 on the right edge, target above (v < 0: -ln 0 in the naive form)
+    ((8, 24, 4, 20), (-3, 20)),     # v == 0 on the upper edge
+    ((8, 24, 4, 20), (40, 4)),      # v == 0 on the lower edge, target to the right (u < 0)
+])
+def test_P0_coincident_gridline_vs_quadrature(rect, tgt):
+    """target on the extension of a cell edge; the modified primitive must give the
+    plain integral (which is regular there)."""
+    unit = 1 / 16
+    K = oracle.cell_kernels(*rect, *tgt, unit)
+    Q = quad_kernels(*(np.array(rect) * unit), tgt[0] * unit, tgt[1] * unit)
+    np.testing.assert_allclose(K, Q, rtol=0, atol=2e-11)
+    for p in ("f80", "f64"):
+        assert np.all(np.isfinite(oracle.cell_kernels(*rect, *tgt, unit, precision=p)))
+
+
+def test_P0_self_cell_offcentre():
+    """Target inside the source cell: cell [0,4]x[0,2], target (1,1). The mirror image [0,2]x[0,2]
+    about the target cancels in K^{x,0}, leaving the regular integral over [2,4]x[0,2]; K^{y,0} = 0."""
+    unit = 1 / 8
+    K = oracle.cell_kernels(0, 32, 0, 16, 8, 8, unit)
+    Q = quad_kernels(2.0, 4.0, 0.0, 2.0, 1.0, 1.0)
+    assert abs(K[0] - Q[0]) < 1e-11
+    assert abs(K[3]) < 1e-15
+    # centred target: both vanish identically (reading A10 of SURVEY.md: no special case needed)
+    K = oracle.cell_kernels(0, 32, 0, 16, 16, 8, unit)
+    assert abs(K[0]) < 1e-17 and abs(K[3]) < 1e-17
+
+
+def test_P0_fig1_grid_forces_vs_quadrature(golden):
+    lay = fig1_layout()
+    r = cell_rects(lay)
+    u = lay.unit
+    # the rebuilt layout is the paper's Table 10 (printed centres are rounded to 2 decimals)
+    rows = golden("paper_table10_leaves.txt")
+    assert lay.n_cells == len(rows) == 28
+    printed = sorted((int(L), float(y), float(x)) for (_id, x, y, L) in rows)
+    mine = sorted((int(l) + 1, float(yc) * u, float(xc) * u) for l, xc, yc in zip(r["level"], r["kxc"], r["kyc"]))
+    for a, b in zip(printed, mine):
+        assert a[0] == b[0] and abs(a[1] - b[1]) <= 0.0051 and abs(a[2] - b[2]) <= 0.0051
+    areas = ((r["kxr"] - r["kxl"]) * (r["kyu"] - r["kyd"])) * u * u
+    assert abs(areas.sum() - 1.0) < 1e-15
+    sig = np.random.default_rng(10).uniform(0.5, 1.5, lay.n_cells)
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"], r["kyc"], u)
+    tsel = [0, 5, 14, 15, 17, 20, 23, 27]          # targets on every level, incl. coarse ones aligned with fine lines
+    for t in tsel:
+        fx = fy = 0.0
+        for c in range(lay.n_cells):
+            if c == t:
+                continue                            # own cell: zero by symmetry (checked above)
+            Q = quad_kernels(r["kxl"][c] * u, r["kxr"][c] * u, r["kyd"][c] * u, r["kyu"][c] * u,
+                             r["kxc"][t] * u, r["kyc"][t] * u)
+            fx += sig[c] * Q[0]
+            fy += sig[c] * Q[3]
+        assert abs(Fx[t] - fx) < 5e-10 and abs(Fy[t] - fy) < 5e-10
+
+
+# ------------------------------------------------------------------------------------------
+# P3: one uniform rectangle
+# ------------------------------------------------------------------------------------------
+def test_P3_single_rectangle_axis_and_far_field():
+    unit = 1 / 32
+    rect = dict(kxl=[-16], kxr=[16], kyd=[-8], kyu=[8])            # [-0.5,0.5] x [-0.25,0.25]
+    A = 1.0 * 0.5
+    # on the x symmetry axis the transverse component vanishes, and the force points at the rectangle
+    Fx, Fy, _ = oracle.force(rect, [2.0], [64, -64, 0, 0], [0, 0, 48, -48], unit, G=3.0)
+    assert abs(Fy[0]) < 1e-16 and abs(Fy[1]) < 1e-16 and abs(Fx[2]) < 1e-16 and abs(Fx[3]) < 1e-16
+    assert Fx[0] < 0 < Fx[1] and Fy[2] < 0 < Fy[3]
+    assert Fx[0] == -Fx[1] and Fy[2] == -Fy[3]
+    # far field -> G sigma A (xc - x)/d^3 (textbook monopole), relative error O(size^2/d^2)
+    for d in (50.0, 200.0):
+        kx, ky = int(round(0.6 * d / unit)), int(round(0.8 * d / unit))
+        x, y = kx * unit, ky * unit
+        dd = math.hypot(x, y)
+        Fx, Fy, _ = oracle.force(rect, [2.0], [kx], [ky], unit, G=3.0)
+        mono = 3.0 * 2.0 * A / dd ** 3
+        assert abs(Fx[0] / (-mono * x) - 1) < 2.0 / dd ** 2
+        assert abs(Fy[0] / (-mono * y) - 1) < 2.0 / dd ** 2
+
+
+# ------------------------------------------------------------------------------------------
+# P4: antisymmetry between equal cells / zero net self-force
+# ------------------------------------------------------------------------------------------
+def test_P4_antisymmetry_and_momentum():
+    unit = 0.5
+    a = dict(kxl=[0], kxr=[2], kyd=[0], kyu=[2])
+    b = dict(kxl=[10], kxr=[12], kyd=[-6], kyu=[-4])
+    Fab = oracle.force(b, [1.0], [1], [1], unit)        # at a's centre from b
+    Fba = oracle.force(a, [1.0], [11], [-5], unit)      # at b's centre from a
+    assert Fab[0][0] == -Fba[0][0] and Fab[1][0] == -Fba[1][0]
+    assert Fab[0][0] > 0 and Fab[1][0] < 0              # attraction towards b (reading R1)
+    lay = uniform_layout(24, -1.0, -1.0, 2 / 24, 1)
+    r = cell_rects(lay)
+    sig = np.random.default_rng(3).uniform(0.1, 2.0, lay.n_cells)
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"], r["kyc"], lay.unit)
+    scale = np.sum(sig * np.hypot(Fx, Fy))
+    assert abs(np.sum(sig * Fx)) < 1e-14 * scale and abs(np.sum(sig * Fy)) < 1e-14 * scale
+
+
+# ------------------------------------------------------------------------------------------
+# P5 / P6: telescoping and refinement invariance on real AMR layouts (exercise the coincidence rule)
+# ------------------------------------------------------------------------------------------
+def test_P5_constant_sigma_telescopes_to_one_rectangle():
+    lay, _ = make_config(2)
+    r = cell_rects(lay)
+    sig = np.full(lay.n_cells, 0.7)
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"], r["kyc"], lay.unit)
+    big = dict(kxl=[r["kxl"].min()], kxr=[r["kxr"].max()], kyd=[r["kyd"].min()], kyu=[r["kyu"].max()])
+    Gx, Gy, _ = oracle.force(big, [0.7], r["kxc"], r["kyc"], lay.unit)
+    assert np.abs(Fx - Gx).max() < 5e-15 and np.abs(Fy - Gy).max() < 5e-15
+
+
+def test_P6_refinement_invariance():
+    """Splitting cells into children that inherit sigma leaves the sum unchanged at every target,
+    including coarse targets that now sit on the extension of fine grid lines."""
+    coarse = uniform_layout(16, -1.0, -1.0, 1 / 8, 1)
+    rc = cell_rects(coarse)
+    sig_c = np.random.default_rng(5).uniform(0.2, 1.0, coarse.n_cells)
+    lay = nested_layout(2, 16, 1.0, 1)                         # central 8x8 refined to 16x16
+    r = cell_rects(lay)
+    # inherit: look up the coarse cell under every leaf (integer geometry; units differ by 2)
+    ci = (r["kxl"] // 4) + 16 * (r["kyd"] // 4)
+    sig = sig_c[ci]
+    tx, ty = 2 * rc["kxc"], 2 * rc["kyc"]                      # coarse centres on the fine lattice
+    keep = ~((np.abs(tx - 32) < 16) & (np.abs(ty - 32) < 16))  # unrefined targets
+    Fx, Fy, _ = oracle.force(r, sig, tx[keep], ty[keep], lay.unit)
+    Gx, Gy, _ = oracle.force(rc, sig_c, rc["kxc"][keep], rc["kyc"][keep], coarse.unit)
+    assert np.abs(Fx - Gx).max() < 1e-14 and np.abs(Fy - Gy).max() < 1e-14
+    # and the refined targets really are on fine grid lines in this test
+    assert np.any((tx[keep] % 2 == 0))
+
+
+# ------------------------------------------------------------------------------------------
+# P1 / P2: the paper's printed tables (readings F3, A13 of SURVEY.md 8(c); R6-R8)
+# ------------------------------------------------------------------------------------------
+def _norms(e, area):
+    return np.sum(np.abs(e) * area), math.sqrt(np.sum(e * e * area)), np.abs(e).max()
+
+
+def _agree_3_digits(val, printed):
+    p = float(printed)
+    return abs(val - p) <= 0.006 * p          # half a unit in the third digit, plus slack for x.xxE-y rounding
+
+
+@pytest.mark.parametrize("Nk", [128, 256])
+def test_P1_paper_table1_D2_uniform(golden, Nk):
+    row = [r for r in golden("paper_table1_D2_uniform.txt") if int(r[0]) == Nk][0]
+    lay = uniform_layout(Nk, -1.0, -1.0, 2 / Nk, 16)
+    r = cell_rects(lay)
+    x, y, h = cell_centres(lay)
+    sig = d2_sigma(x, y, 0.5)
+    dx, dy = d2_slopes(x, y, 0.5)
+    q = np.nonzero((x > 0) & (y > 0))[0]            # one quadrant; the disk is mirror-symmetric
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+    ax, ay = F_D2_xy(x[q], y[q], 0.5)
+    R = np.hypot(x[q], y[q])
+    ex = Fx - ax
+    eR = (Fx * x[q] + Fy * y[q]) / R - (ax * x[q] + ay * y[q]) / R
+    A = 4 * h[q] ** 2
+    got = list(_norms(ex, A)) + list(_norms(eR, A))
+    for g, p in zip(got, row[1:]):
+        assert _agree_3_digits(g, p), (got, row)
+
+
+def test_P1_paper_table2_D22_uniform(golden):
+    row = [r for r in golden("paper_table2_D22_uniform.txt") if int(r[0]) == 128][0]
+    lay = uniform_layout(128, -1.0, -1.0, 2 / 128, 16)
+    r = cell_rects(lay)
+    x, y, h = cell_centres(lay)
+    sig = d22_sigma(x, y)
+    dx, dy = d22_slopes(x, y)
+    q = np.nonzero((x > 0) & (y > 0))[0]
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+    a1 = F_D2_xy(x[q], y[q], 0.4, 0.0, 0.5)
+    a2 = F_D2_xy(x[q], y[q], 0.4, 0.0, -0.5)
+    A = 4 * h[q] ** 2
+    got = list(_norms(Fx - a1[0] - a2[0], A)) + list(_norms(Fy - a1[1] - a2[1], A))
+    for g, p in zip(got, row[1:]):
+        assert _agree_3_digits(g, p), (got, row)
+
+
+@pytest.mark.parametrize("L,Nk", [(2, 128), (3, 128)])
+def test_P2_paper_table3_ILR_Linf(golden, L, Nk):
+    """AMR pin: needs the coincidence rule of PAPER.md:98 on a real quadtree."""
+    row = [r for r in golden("paper_table3_ILR_Linf.txt") if int(r[0]) == L and int(r[1]) == Nk][0]
+    lay = paper_ilr_layout(Nk, L, "D2")
+    r = cell_rects(lay)
+    x, y, h = cell_centres(lay)
+    sig = d2_sigma(x, y, 0.5)
+    dx, dy = d2_slopes(x, y, 0.5)
+    q = np.nonzero((x > 0) & (y > 0))[0]
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+    ax, ay = F_D2_xy(x[q], y[q], 0.5)
+    R = np.hypot(x[q], y[q])
+    assert _agree_3_digits(np.abs(Fx - ax).max(), row[2])
+    assert _agree_3_digits(np.abs((Fx * x[q] + Fy * y[q]) / R - (ax * x[q] + ay * y[q]) / R).max(), row[3])
+
+
+def test_paper_leaf_counts_tables_8_9(golden):
+    for rule, disk, L, Nk, EL in golden("paper_table8_9_leaf_counts.txt"):
+        if int(Nk) > 256:
+            continue
+        f = paper_ilr_layout if rule == "ILR" else paper_vlr_layout
+        assert f(int(Nk), int(L), disk).n_cells == int(EL), (rule, disk, L, Nk)
+
+
+# ------------------------------------------------------------------------------------------
+# P8: convergence (north_star pin (d) as it can hold: SURVEY.md 8(c) F1, F2; R11)
+# ------------------------------------------------------------------------------------------
+def test_P8_D2_order_of_accuracy():
+    """sigma^0 only is first order; with the Taylor slopes of Eq. 6 it is second order (L1 norm)."""
+    e0, e1 = [], []
+    for Nk in (32, 64, 128):
+        lay = uniform_layout(Nk, -1.0, -1.0, 2 / Nk, 16)
+        r = cell_rects(lay)
+        x, y, h = cell_centres(lay)
+        q = np.nonzero((x > 0) & (y > 0))[0]
+        sig = d2_sigma(x, y, 0.5)
+        dx, dy = d2_slopes(x, y, 0.5)
+        ax, _ = F_D2_xy(x[q], y[q], 0.5)
+        A = 4 * h[q] ** 2
+        F0, _, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, precision="f64")
+        F1, _, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+        e0.append(np.sum(np.abs(F0 - ax) * A))
+        e1.append(np.sum(np.abs(F1 - ax) * A))
+    o0 = [math.log2(e0[i] / e0[i + 1]) for i in range(2)]
+    o1 = [math.log2(e1[i] / e1[i + 1]) for i in range(2)]
+    assert all(0.85 < o < 1.2 for o in o0), o0
+    assert all(1.8 < o < 2.2 for o in o1), o1
+
+
+def test_P8_kuzmin_nested_convergence():
+    """Analytic Kuzmin mid-plane force -G M R/(R^2+a^2)^{3/2} (north_star pin (d)), on a nested grid
+    reaching |x| <= 256 so that the truncated mass is negligible.  sigma^0 only: order ~ 1."""
+    errs = []
+    for n in (16, 32):
+        lay = nested_layout(9, n, 256.0, n // 4)
+        r = cell_rects(lay)
+        x, y, h = cell_centres(lay)
+        sig = kuzmin_sigma(x, y, 1.0, 0.2)
+        inner = np.nonzero((np.abs(x) < 1) & (np.abs(y) < 1) & (x > 0) & (y > 0))[0]
+        Fx, Fy, _ = oracle.force(r, sig, r["kxc"][inner], r["kyc"][inner], lay.unit, precision="f64")
+        R2 = x[inner] ** 2 + y[inner] ** 2
+        ax = -x[inner] / (R2 + 0.04) ** 1.5
+        ay = -y[inner] / (R2 + 0.04) ** 1.5
+        fmax = np.max(np.hypot(ax, ay))
+        errs.append(max(np.abs(Fx - ax).max(), np.abs(Fy - ay).max()) / fmax)
+        assert np.all(np.isfinite(Fx)) and np.all(np.isfinite(Fy))
+    order = math.log2(errs[0] / errs[1])
+    assert errs[1] < 0.25 and 0.8 < order < 1.6, (errs, order)
