@@ -1,0 +1,134 @@
+/*
+ * sg_disk.h -- C ABI of the B200 (sm_100a) direct self-gravity library for a razor-thin disk on
+ * block-structured AMR, after arXiv 2001.02765 (Tseng, Shang & Yen).  Citations are lines of
+ * /root/reference/PAPER.md (the paper's text) with the section / equation they fall in.
+ *
+ * What the library computes (PAPER.md:57-69 Eq. 4-5, :86-94, :96-100, :104, :110; readings in DESIGN.md):
+ * the domain is the disjoint union of axis-aligned leaf cells D_c = [x_l,x_r] x [y_d,y_u], each carrying
+ * one surface density sigma_c (the zeroth-order Taylor coefficient of Eq. 6).  At the centre (x_t,y_t)
+ * of EVERY leaf cell t
+ *
+ *     Fx_t = G * sum_c sigma_c * K_c^{x,0}(x_t,y_t),      Fy_t = G * sum_c sigma_c * K_c^{y,0}(x_t,y_t)
+ *
+ * where K_c^{x,0} = integral over D_c of (xbar-x_t)/r^3 = [[ -ln( (ybar-y_t) + r ) ]] is the closed-form
+ * mixed corner difference of PAPER.md:90-94 (z = 0), K^{y,0} the same with x and y exchanged, and where
+ * a target that lies on the extension of a source grid line (xbar == x_t, exact on the integer
+ * lattice) uses the paper's modified primitive.  The sum runs over ALL leaves,
+ * the target's own cell included.  Everything is FP64.
+ *
+ * Conventions
+ *   - return value: SG_OK (0) or a negative SG_ERR_* code; sg_last_error() gives a message.
+ *   - levels: level 0 is the coarsest; cell_width[l+1] == cell_width[l] / 2.
+ *   - a patch is P x P leaf cells of one level; (level, i0, j0) is the index of its lower-left cell on
+ *     that level's lattice counted from (x0, y0); i0 and j0 must be multiples of P.  Only LEAF patches
+ *     are listed (a refined patch is replaced by its four children).
+ *   - cell order, used by sigma, Fx, Fy and sg_cell_geometry: [patch][j][i], i (x) fastest, patches in
+ *     the order given to sg_create.
+ *   - "host" / "device" below says where a pointer must live.  The context never frees or keeps a
+ *     caller pointer beyond the call (device work is enqueued on the caller's stream and reads/writes
+ *     the caller's device buffers asynchronously: keep them alive until the stream has drained).
+ *   - there is no CPU fallback: every call that computes runs CUDA kernels on the context's device.
+ */
+#ifndef SG_DISK_H
+#define SG_DISK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SG_OK          0
+#define SG_ERR_ARG    -1   /* null pointer, non-positive size, widths not halving, ...            */
+#define SG_ERR_LAYOUT -2   /* patch off its lattice / overlapping / duplicate / too large          */
+#define SG_ERR_CUDA   -3   /* a CUDA runtime call failed (message has the CUDA error string)       */
+#define SG_ERR_STATE  -4   /* sg_force before sg_set_density                                       */
+
+typedef struct sg_ctx sg_ctx;                        /* opaque; owns every device array of the layout */
+typedef struct { int32_t level, i0, j0; } sg_patch;  /* lower-left cell of a P x P leaf patch          */
+
+/*
+ * S1, layout build (PAPER.md:57-67: the D_i are disjoint rectangles; :104-110: leaf zones and their
+ * centres).  Host work + uploads; synchronous.  Validates the patch list (levels in range, i0/j0 >= 0
+ * and multiples of P, no duplicate, no patch inside another -> SG_ERR_LAYOUT), puts every cell edge
+ * and centre on one integer lattice of unit cell_width[n_levels-1]/2, deduplicates cell corners
+ * into a global vertex list with the <= 4 signed adjacent cells of each, and builds the per-column /
+ * per-row tables used by the coincidence-safe separable part ("Kernels").
+ *   out            host, receives the context
+ *   cell_width     host [n_levels], physical widths; only cell_width[n_levels-1] enters the result
+ *   x0, y0         physical lower-left corner of the level-0 lattice (reported back by sg_cell_geometry;
+ *                  forces are translation invariant)
+ *   patch_cells    P >= 1
+ *   leaf_patches   host [n_patches], copied
+ *   G              gravitational constant multiplying the sums (PAPER.md:139 uses G = 1)
+ *   device         CUDA device ordinal
+ * 2:1 balance is NOT required by the sum (any disjoint cover is valid, e.g. the paper's Table 10
+ * example); sg_layout_info reports whether the layout is balanced.
+ */
+int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, double y0,
+              int patch_cells, const sg_patch *leaf_patches, int64_t n_patches, double G, int device);
+
+void sg_destroy(sg_ctx *ctx);                        /* frees device and host memory; NULL is allowed */
+
+int64_t sg_num_cells(const sg_ctx *ctx);             /* N = n_patches * P * P ; -1 on NULL            */
+int64_t sg_num_vertices(const sg_ctx *ctx);          /* N_v, deduplicated cell corners                */
+
+/* info[0]=N, [1]=N_v, [2]=#distinct vertex x, [3]=#distinct vertex y, [4]=#distinct target x,
+ * [5]=#distinct target y, [6]=1 if 2:1 balanced across faces and corners else 0, [7]=bytes of device
+ * memory held by the context.  info: host [8]. */
+int sg_layout_info(const sg_ctx *ctx, int64_t *info);
+
+/* Cell centres and widths in physical units, library cell order.  xc, yc, h: host [N], any may be NULL. */
+int sg_cell_geometry(const sg_ctx *ctx, double *xc, double *yc, double *h);
+
+/*
+ * S2, sigma -> signed vertex weights (exact regrouping of the corner differences of PAPER.md:92-94:
+ * sum_c sigma_c [[P]]_c = sum_v w_v P(v), w_v = sum over the cells that have v as a corner of
+ * +sigma (NE or SW corner) / -sigma (NW or SE corner)), plus the per-column / per-row cumulative
+ * weights of the separable part.   sigma_dev: device [N], library cell order, FP64.   Asynchronous on
+ * cuda_stream (a cudaStream_t passed as void*, NULL = default stream).
+ */
+int sg_set_density(sg_ctx *ctx, const double *sigma_dev, void *cuda_stream);
+
+/*
+ * S3-S5, the all-pairs sum.  Fx_dev, Fy_dev: device [N] (or [count] when a
+ * target range is set, see below), FP64, written in library cell order.  Asynchronous on
+ * cuda_stream.  Deterministic: the same context and sigma give bit-identical results run to run
+ * (no floating-point atomics).  SG_ERR_STATE if no density has been set.
+ */
+int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
+
+/*
+ * Restrict sg_force to the targets [first, first+count) of the library cell order (all sources are
+ * still summed).  Fx_dev/Fy_dev then hold count values.  This is how the path shards over GPUs:
+ * targets are independent, each rank owns a slice, no collective is needed.
+ * count == 0 is allowed (sg_force does nothing).  Default: first = 0, count = N.
+ */
+int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
+
+/* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
+int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
+
+/* Device time of the most recent sg_force interaction kernel launch is not recorded by the library;
+ * callers time with their own events.  This diagnostic enqueues only the interaction kernel (S3)
+ * on cuda_stream, between two events it owns, synchronises, and returns its duration in ms.  Used by
+ * bench.py for the roofline line. */
+int sg_time_interaction_kernel(sg_ctx *ctx, void *cuda_stream, float *ms);
+
+/* FP64-pipe instructions (warp-level, per (target, vertex) pair) and FP64 FLOPs per pair of the
+ * interaction kernel as built (counted from its SASS); vertex evaluations per
+ * sg_force with the current target range.  Any pointer may be NULL. */
+int sg_kernel_model(const sg_ctx *ctx, double *fp64_instr_per_pair, double *flops_per_pair,
+                    double *pair_evaluations);
+
+/* Diagnostic: sustained DFMA rate of the device (8 independent chains per thread, full occupancy),
+ * in FP64 TFLOP/s (FMA = 2), and the same as warp-instructions/s.  Synchronous. */
+int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s);
+
+const char *sg_last_error(const sg_ctx *ctx);        /* ctx may be NULL: error of the last failed sg_create */
+const char *sg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SG_DISK_H */

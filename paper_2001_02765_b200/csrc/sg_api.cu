@@ -1,0 +1,300 @@
+// sg_api.cu -- the C ABI of include/sg_disk.h: context ownership, uploads, launch planning.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "sg_kernels.cuh"
+#include "sg_layout.h"
+
+using namespace sg;
+
+struct sg_ctx {
+    HostLayout host;
+    DevLayout dev;
+    int device = -1;             // < 0: host-only context (layout queries work, compute calls fail)
+    int sm_count = 148;
+    bool density_set = false;
+    int64_t first = 0, count = 0;
+    int64_t dev_bytes = 0;
+    std::vector<void *> allocs;
+    std::string err;
+};
+
+static thread_local std::string g_create_error;
+
+namespace {
+
+#define SG_CUDA(ctx, call)                                                              \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess) {                                                        \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);            \
+            return SG_ERR_CUDA;                                                         \
+        }                                                                               \
+    } while (0)
+
+template <class T>
+int dev_alloc(sg_ctx *c, T **p, int64_t n) {
+    const size_t bytes = size_t(std::max<int64_t>(n, 1)) * sizeof(T);
+    SG_CUDA(c, cudaMalloc(reinterpret_cast<void **>(p), bytes));
+    c->allocs.push_back(*p);
+    c->dev_bytes += int64_t(bytes);
+    return SG_OK;
+}
+
+template <class T>
+int upload(sg_ctx *c, T **p, const std::vector<T> &h) {
+    int rc = dev_alloc(c, p, int64_t(h.size()));
+    if (rc) return rc;
+    if (!h.empty()) SG_CUDA(c, cudaMemcpy(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return SG_OK;
+}
+
+// Work items = target blocks x source splits, walked round-robin by a persistent grid of
+// 2 CTAs per SM.  Pick the split count that keeps the last round of items fullest.
+ForcePlan make_plan(const sg_ctx *c) {
+    ForcePlan p;
+    p.first = c->first; p.count = c->count;
+    p.smem = interaction_smem_bytes(c->dev.tab_entries);
+    if (p.count == 0) return p;
+    p.T = p.count > 16384 ? 4 : 1;
+    const int64_t per_block = int64_t(kThreads) * p.T;
+    p.n_tblocks = int((p.count + per_block - 1) / per_block);
+    const int slots = c->sm_count * 2;
+    const int n_tiles = c->dev.n_tiles;
+    int best_split = 1; double best_eff = -1.0;
+    const int want = std::max(1, std::min(n_tiles, (4 * slots + p.n_tblocks - 1) / p.n_tblocks));
+    for (int s = want; s <= std::min(n_tiles, want + 12); ++s) {
+        const int tps = (n_tiles + s - 1) / s, ns = (n_tiles + tps - 1) / tps;
+        const int64_t items = int64_t(ns) * p.n_tblocks;
+        const int64_t rounds = (items + slots - 1) / slots;
+        // cost ~ rounds * tiles per item; ideal ~ items * tps / slots
+        const double eff = double(n_tiles) * p.n_tblocks / (double(rounds) * slots * tps);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best_split = ns; }
+    }
+    p.tiles_per_split = (n_tiles + best_split - 1) / best_split;
+    p.n_split = (n_tiles + p.tiles_per_split - 1) / p.tiles_per_split;
+    const int64_t items = int64_t(p.n_split) * p.n_tblocks;
+    p.grid = int(std::min<int64_t>(items, slots));
+    return p;
+}
+
+int ensure_partials(sg_ctx *c, const ForcePlan &p) {
+    const int64_t need = int64_t(p.n_split) * 2 * p.count;
+    if (need <= c->dev.part_capacity) return SG_OK;
+    if (c->dev.part) {
+        SG_CUDA(c, cudaDeviceSynchronize());
+        cudaFree(c->dev.part);
+        c->allocs.erase(std::remove(c->allocs.begin(), c->allocs.end(), (void *)c->dev.part), c->allocs.end());
+        c->dev_bytes -= c->dev.part_capacity * 8;
+        c->dev.part = nullptr; c->dev.part_capacity = 0;
+    }
+    int rc = dev_alloc(c, &c->dev.part, need);
+    if (rc) return rc;
+    c->dev.part_capacity = need;
+    return SG_OK;
+}
+
+int upload_layout(sg_ctx *c) {
+    const HostLayout &h = c->host;
+    DevLayout &d = c->dev;
+    d.N = h.N; d.Nv = h.Nv;
+    d.nX = int(h.colX.size()); d.nY = int(h.rowY.size());
+    d.ntX = int(h.tX.size()); d.ntY = int(h.tY.size());
+    d.n_tiles = int((h.Nv + kTile - 1) / kTile);
+    const int64_t tb_bytes = (int64_t(d.ntY) * d.nX + int64_t(d.ntX) * d.nY) * 8;
+    if (tb_bytes > (int64_t(48) << 30)) {
+        c->err = "line tables would need more than 48 GiB: layout too large for this build";
+        return SG_ERR_LAYOUT;
+    }
+    std::vector<double2> tgt(size_t(h.N));
+    for (int64_t i = 0; i < h.N; ++i) tgt[i] = make_double2(double(h.tkx[i]), double(h.tky[i]));
+    int rc;
+    if ((rc = upload(c, &d.tgt, tgt))) return rc;
+    if ((rc = upload(c, &d.itx, h.itx)) || (rc = upload(c, &d.ity, h.ity))) return rc;
+    if ((rc = upload(c, &d.adj, h.adj))) return rc;
+    if ((rc = upload(c, &d.vkx, h.vkx)) || (rc = upload(c, &d.vky, h.vky))) return rc;
+    if ((rc = upload(c, &d.colX, h.colX)) || (rc = upload(c, &d.colstart, h.colstart))) return rc;
+    if ((rc = upload(c, &d.rowY, h.rowY)) || (rc = upload(c, &d.rowstart, h.rowstart))) return rc;
+    if ((rc = upload(c, &d.rowperm, h.rowperm))) return rc;
+    if ((rc = upload(c, &d.tX, h.tX)) || (rc = upload(c, &d.tY, h.tY))) return rc;
+    if ((rc = dev_alloc(c, &d.vtile, int64_t(d.n_tiles) * kTileDoubles))) return rc;
+    if ((rc = dev_alloc(c, &d.w, h.Nv))) return rc;
+    if ((rc = dev_alloc(c, &d.TBx, int64_t(d.ntY) * d.nX))) return rc;
+    if ((rc = dev_alloc(c, &d.TBy, int64_t(d.ntX) * d.nY))) return rc;
+
+    // log-table range: arguments a = |v| + r with r >= 1 (a target never sits on a vertex) and
+    // a <= (1 + sqrt 2) * extent, all in lattice units.
+    const double a_max = 2.5 * double(h.extent) + 2.0;
+    int e_max = 0;
+    std::frexp(a_max, &e_max);                       // a_max < 2^e_max
+    d.tab_idx0 = 0x3ff << kLogK;                     // a = 1.0
+    d.tab_entries = (e_max + 1) << kLogK;
+    if ((rc = dev_alloc(c, &d.lntab, d.tab_entries))) return rc;
+    SG_CUDA(c, configure_kernels(d.tab_entries));
+    launch_build_logtab(d, nullptr);
+    launch_fill_static_tiles(d, nullptr);
+    SG_CUDA(c, cudaGetLastError());
+    SG_CUDA(c, cudaDeviceSynchronize());
+    return SG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, double y0, int patch_cells,
+              const sg_patch *leaf_patches, int64_t n_patches, double G, int device) {
+    if (!out) { g_create_error = "out is NULL"; return SG_ERR_ARG; }
+    *out = nullptr;
+    if (!std::isfinite(G)) { g_create_error = "G must be finite"; return SG_ERR_ARG; }
+    sg_ctx *c = new sg_ctx();
+    int rc = build_layout(c->host, n_levels, cell_width, x0, y0, patch_cells, leaf_patches, n_patches, c->err);
+    if (rc == SG_OK) {
+        c->device = device;
+        c->dev.G = G;
+        c->first = 0; c->count = c->host.N;
+        if (device >= 0) {
+            cudaError_t e = cudaSetDevice(device);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+            if (e != cudaSuccess) {
+                c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(e);
+                rc = SG_ERR_CUDA;
+            } else {
+                rc = upload_layout(c);
+            }
+        }
+    }
+    if (rc != SG_OK) {
+        g_create_error = c->err;
+        sg_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return SG_OK;
+}
+
+void sg_destroy(sg_ctx *c) {
+    if (!c) return;
+    if (c->device >= 0) {
+        cudaSetDevice(c->device);
+        cudaDeviceSynchronize();
+        for (void *p : c->allocs) cudaFree(p);
+    }
+    delete c;
+}
+
+int64_t sg_num_cells(const sg_ctx *c) { return c ? c->host.N : -1; }
+int64_t sg_num_vertices(const sg_ctx *c) { return c ? c->host.Nv : -1; }
+
+int sg_layout_info(const sg_ctx *c, int64_t *info) {
+    if (!c || !info) return SG_ERR_ARG;
+    info[0] = c->host.N; info[1] = c->host.Nv;
+    info[2] = int64_t(c->host.colX.size()); info[3] = int64_t(c->host.rowY.size());
+    info[4] = int64_t(c->host.tX.size()); info[5] = int64_t(c->host.tY.size());
+    info[6] = c->host.balanced ? 1 : 0;
+    info[7] = c->dev_bytes;
+    return SG_OK;
+}
+
+int sg_cell_geometry(const sg_ctx *c, double *xc, double *yc, double *h) {
+    if (!c) return SG_ERR_ARG;
+    const HostLayout &L = c->host;
+    const int64_t PP = int64_t(L.P) * L.P;
+    for (int64_t i = 0; i < L.N; ++i) {
+        if (xc) xc[i] = L.x0 + double(L.tkx[i]) * L.unit;
+        if (yc) yc[i] = L.y0 + double(L.tky[i]) * L.unit;
+        if (h) h[i] = L.unit * double(int64_t(2) << (L.n_levels - 1 - L.patches[i / PP].level));
+    }
+    return SG_OK;
+}
+
+int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
+    if (!c) return SG_ERR_ARG;
+    if (!sigma_dev) { c->err = "sigma_dev is NULL"; return SG_ERR_ARG; }
+    if (c->device < 0) { c->err = "host-only context (device < 0): no CUDA path, and there is no CPU fallback"; return SG_ERR_CUDA; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    SG_CUDA(c, cudaSetDevice(c->device));
+    launch_vertex_weights(c->dev, sigma_dev, s);
+    launch_line_tables(c->dev, s);
+    SG_CUDA(c, cudaGetLastError());
+    c->density_set = true;
+    return SG_OK;
+}
+
+int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
+    if (!c) return SG_ERR_ARG;
+    if (c->device < 0) { c->err = "host-only context (device < 0): no CUDA path, and there is no CPU fallback"; return SG_ERR_CUDA; }
+    if (!c->density_set) { c->err = "sg_force called before sg_set_density"; return SG_ERR_STATE; }
+    if (c->count == 0) return SG_OK;
+    if (!Fx_dev || !Fy_dev) { c->err = "Fx_dev / Fy_dev is NULL"; return SG_ERR_ARG; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    SG_CUDA(c, cudaSetDevice(c->device));
+    const ForcePlan p = make_plan(c);
+    int rc = ensure_partials(c, p);
+    if (rc) return rc;
+    launch_interaction(c->dev, p, s);
+    launch_finalise(c->dev, p, Fx_dev, Fy_dev, s);
+    SG_CUDA(c, cudaGetLastError());
+    return SG_OK;
+}
+
+int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
+    if (!c) return SG_ERR_ARG;
+    if (first < 0 || count < 0 || first + count > c->host.N) {
+        c->err = "target range outside [0, N)"; return SG_ERR_ARG;
+    }
+    c->first = first; c->count = count;
+    return SG_OK;
+}
+
+int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
+    if (!c) return SG_ERR_ARG;
+    if (set_density_launches) *set_density_launches = 3;      // vertex weights, column table, row table
+    if (force_launches) *force_launches = c->count > 0 ? 2 : 0;   // interaction, finalise
+    return SG_OK;
+}
+
+int sg_time_interaction_kernel(sg_ctx *c, void *cuda_stream, float *ms) {
+    if (!c || !ms) return SG_ERR_ARG;
+    if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
+    if (!c->density_set) { c->err = "no density set"; return SG_ERR_STATE; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    SG_CUDA(c, cudaSetDevice(c->device));
+    const ForcePlan p = make_plan(c);
+    int rc = ensure_partials(c, p);
+    if (rc) return rc;
+    cudaEvent_t e0, e1;
+    SG_CUDA(c, cudaEventCreate(&e0));
+    SG_CUDA(c, cudaEventCreate(&e1));
+    SG_CUDA(c, cudaEventRecord(e0, s));
+    launch_interaction(c->dev, p, s);
+    SG_CUDA(c, cudaEventRecord(e1, s));
+    SG_CUDA(c, cudaEventSynchronize(e1));
+    SG_CUDA(c, cudaEventElapsedTime(ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    SG_CUDA(c, cudaGetLastError());
+    return SG_OK;
+}
+
+int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_per_pair, double *pair_evaluations) {
+    if (!c) return SG_ERR_ARG;
+    if (fp64_instr_per_pair) *fp64_instr_per_pair = kFp64InstrPerPair;
+    if (flops_per_pair) *flops_per_pair = kFlopsPerPair;
+    if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);
+    return SG_OK;
+}
+
+int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s) {
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = measure_dfma(tflops, warp_instr_per_s);
+    if (e != cudaSuccess) { g_create_error = std::string("sg_measure_fp64_peak: ") + cudaGetErrorString(e); return SG_ERR_CUDA; }
+    return SG_OK;
+}
+
+const char *sg_last_error(const sg_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+const char *sg_version(void) { return "sg-disk-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,43 @@
+// sg_layout.h -- internal: host-side flattened AMR layout (S1 of DESIGN.md).  Not part of the C ABI.
+//
+// All coordinates are integers on one lattice whose unit is half the finest cell width, so every
+// cell edge (even multiples of 2^(L-1-level)) and every cell centre is an integer and the paper's
+// coincidence test "xbar == x" (sgn(|xbar-x|)) is an exact integer comparison.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/sg_disk.h"
+
+namespace sg {
+
+constexpr int32_t kMaxLattice = 1 << 26;   // u^2+v^2 < 2^53 stays an exact FP64 integer
+
+struct HostLayout {
+    int n_levels = 0, P = 0;
+    double unit = 0.0, x0 = 0.0, y0 = 0.0;
+    int64_t N = 0, Nv = 0;
+    int32_t extent = 0;                    // max lattice coordinate of any vertex (>= 2)
+    bool balanced = true;
+    std::vector<sg_patch> patches;
+
+    // targets (leaf-cell centres), library cell order [patch][j][i]
+    std::vector<int32_t> tkx, tky;         // lattice coordinates
+    std::vector<int32_t> itx, ity;         // index into tX / tY
+    std::vector<int32_t> tX, tY;           // sorted distinct target x / y
+
+    // vertices (deduplicated cell corners), sorted by (kx, ky): column c is the contiguous range
+    // [colstart[c], colstart[c+1]) and is sorted by ky inside.
+    std::vector<int32_t> vkx, vky;
+    std::vector<int32_t> adj;              // [4*Nv]: (cell << 1) | neg, or -1; neg=1 for NW / SE corners
+    std::vector<int32_t> colX, colstart;   // distinct vertex x (sorted); [nX+1]
+    std::vector<int32_t> rowY, rowstart;   // distinct vertex y (sorted); [nY+1]
+    std::vector<int32_t> rowperm;          // vertex indices sorted by (ky, kx)
+};
+
+// Returns SG_OK or SG_ERR_*; on error `err` holds the message.
+int build_layout(HostLayout &out, int n_levels, const double *cell_width, double x0, double y0,
+                 int P, const sg_patch *patches, int64_t n_patches, std::string &err);
+
+}  // namespace sg
