@@ -28,3 +28,11 @@ def read_golden(name):
 @pytest.fixture(scope="session")
 def golden():
     return read_golden
+
+
+def pytest_sessionstart(session):
+    """Build the in-tree CUDA library (nvcc cross-compiles without a GPU) and the C oracle once."""
+    from paper_2001_02765_b200.build import build as build_lib
+    from oracle.build import build as build_oracle
+    build_lib()
+    build_oracle()

@@ -1,0 +1,133 @@
+"""CPU-side tests of the C-ABI library: it loads, exports every symbol include/sg_disk.h declares,
+and the host layout builder (S1) validates and flattens patch lists correctly.  No compute calls:
+contexts are created with device = -1 (host-only), on which every compute entry must fail loudly."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2001_02765_b200 as sgd
+from paper_2001_02765_b200 import SgDisk, SgError, binding
+from workloads import Layout, make_config, cell_rects, expected_counts, paper_ilr_layout
+from workloads.configs import cell_centres, _sorted_patches, uniform_layout
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "sg_disk.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sg_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTED_SYMBOLS)
+    lib = ctypes.CDLL(binding.lib_path())
+    for name in declared:
+        assert getattr(lib, name) is not None
+    assert "sm_100a" in sgd.version()
+
+
+def test_no_oracle_in_product_path():
+    """The product package must not import, read or link anything under oracle/ (or _work/)."""
+    pkg = os.path.join(ROOT, "paper_2001_02765_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.lower(), f"{f} mentions the oracle"
+                assert "_work" not in src, f
+
+
+@pytest.mark.parametrize("cfg,n_v", [(1, 65 * 65), (2, 7361), (3, 53889)])
+def test_layout_counts_and_geometry(cfg, n_v):
+    lay, _ = make_config(cfg)
+    exp = expected_counts(cfg)
+    with SgDisk.from_layout(lay, device=-1) as d:
+        info = d.layout_info()
+        assert info["n_cells"] == exp["n_cells"] == d.num_cells
+        assert info["n_vertices"] == n_v == d.num_vertices          # SURVEY.md section 8 size table
+        assert info["balanced"] == 1
+        xc, yc, h = d.cell_geometry()
+    x, y, hh = cell_centres(lay)
+    assert np.array_equal(xc, x) and np.array_equal(yc, y) and np.array_equal(h, hh)
+
+
+def test_vertex_count_matches_bruteforce_dedupe():
+    lay = paper_ilr_layout(32, 3)                     # P = 1 quadtree of the paper's kind, with hanging nodes
+    r = cell_rects(lay)
+    corners = set()
+    for a, b in (("kxl", "kyd"), ("kxl", "kyu"), ("kxr", "kyd"), ("kxr", "kyu")):
+        corners |= set(zip(r[a].tolist(), r[b].tolist()))
+    with SgDisk.from_layout(lay, device=-1) as d:
+        assert d.num_vertices == len(corners)
+        assert d.num_cells == lay.n_cells
+
+
+def test_unbalanced_layout_is_accepted_and_flagged():
+    # Fig. 1 / Table 10 of the paper: level-3 zones abut a level-1 zone
+    l0 = [(0, i, j) for j in range(4) for i in range(4) if (i, j) not in ((1, 1), (2, 2))]
+    l1 = [(1, 2, 2), (1, 3, 3)] + [(1, 4 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]
+    l2 = [(2, 4 + di, 6 + dj) for dj in (0, 1) for di in (0, 1)]
+    l2 += [(2, 6 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]
+    lay = Layout(3, np.array([0.25, 0.125, 0.0625]), 0.0, 0.0, 1, _sorted_patches(l0 + l1 + l2))
+    with SgDisk.from_layout(lay, device=-1) as d:
+        assert d.num_cells == 28                       # "28 leaves"
+        assert d.layout_info()["balanced"] == 0
+        _, _, h = d.cell_geometry()
+        assert abs(np.sum(h * h) - 1.0) < 1e-15        # leaves tile [0,1]^2
+
+
+def test_layout_errors():
+    lay, _ = make_config(2)
+    mk = lambda **kw: SgDisk(kw.get("nl", lay.n_levels), kw.get("cw", lay.cell_width), -1, -1, kw.get("P", lay.P),
+                             kw.get("p", lay.patches), device=-1)
+    with pytest.raises(SgError) as e:                  # fine patch inside a coarse leaf
+        mk(p=np.vstack([lay.patches, [[1, 0, 0]]]))
+    assert e.value.code == binding.SG_ERR_LAYOUT and "overlap" in str(e.value)
+    with pytest.raises(SgError) as e:                  # coarse patch over existing fine leaves
+        mk(p=np.vstack([lay.patches, [[0, 16, 16]]]))
+    assert e.value.code == binding.SG_ERR_LAYOUT
+    with pytest.raises(SgError) as e:                  # duplicate
+        mk(p=np.vstack([lay.patches, lay.patches[:1]]))
+    assert e.value.code == binding.SG_ERR_LAYOUT and "duplicate" in str(e.value)
+    with pytest.raises(SgError) as e:                  # off the patch lattice
+        mk(p=np.array([[0, 3, 0]], dtype=np.int32))
+    assert e.value.code == binding.SG_ERR_LAYOUT
+    with pytest.raises(SgError) as e:                  # level out of range
+        mk(p=np.array([[2, 0, 0]], dtype=np.int32))
+    assert e.value.code == binding.SG_ERR_LAYOUT
+    with pytest.raises(SgError) as e:                  # widths not halving
+        mk(cw=[1 / 32, 1 / 48])
+    assert e.value.code == binding.SG_ERR_ARG
+    with pytest.raises(SgError) as e:
+        mk(P=0)
+    assert e.value.code == binding.SG_ERR_ARG
+    with pytest.raises(SgError) as e:                  # lattice too large for exact FP64 integers
+        SgDisk(1, [1.0], 0, 0, 16, np.array([[0, 1 << 25, 0]], dtype=np.int32), device=-1)
+    assert e.value.code == binding.SG_ERR_LAYOUT
+
+
+def test_host_only_context_never_computes():
+    """No CPU fallback: compute entry points on a context without a device return SG_ERR_CUDA."""
+    lay = uniform_layout(16, 0.0, 0.0, 1.0, 8)
+    with SgDisk.from_layout(lay, device=-1) as d:
+        lib = binding.load_library()
+        dummy = ctypes.c_void_p(16)
+        assert lib.sg_set_density(d._ctx, dummy, None) == binding.SG_ERR_CUDA
+        assert lib.sg_force(d._ctx, dummy, dummy, None) == binding.SG_ERR_CUDA
+        assert b"no CPU fallback" in lib.sg_last_error(d._ctx)
+        assert d.launch_counts() == (3, 2)
+        d.set_target_range(5, 0)
+        assert d.launch_counts() == (3, 0)
+        with pytest.raises(SgError):
+            d.set_target_range(250, 10)
+
+
+def test_shard_range_partitions_targets():
+    for n in (0, 1, 7, 4096, 1048576, 448768):
+        for world in (1, 2, 3, 8):
+            pieces = [binding.shard_range(n, r, world) for r in range(world)]
+            assert pieces[0][0] == 0 and sum(c for _, c in pieces) == n
+            for (f0, c0), (f1, _) in zip(pieces, pieces[1:]):
+                assert f0 + c0 == f1
+            assert max(c for _, c in pieces) - min(c for _, c in pieces) <= 1
