@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for BASELINE.json's metric: FP64 cell-pair interactions/s per Fx,Fy evaluation.
+
+A "step" is one pass of the whole hot path over one density field: sg_set_density (S2: vertex weights +
+line tables) then sg_force (S3 interaction kernel, S4/S5 finalise).  Workload at N = 1 GPU: BASELINE.json
+config 5 (uniform 1024 x 1024, 1,048,576 leaves, 1.1e12 pairs per evaluation), the >= 1 M-cell case the
+north_star bar is quoted on.  With N > 1 GPUs the targets are sharded across ranks (targets are
+independent; :265: "12 cards"), every rank sums over all sources, no data-path collective: strong scaling.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "FP64 cell-pair interactions/s per Fx,Fy evaluation"
+UNIT = "pairs/s"
+# Nominal FP64 peak used as the roofline denominator: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+# (SM count and max SM clock from /opt/skills/guides/B200_PROFILING.md; 64 lanes/SM = 4 sub-partitions x 16,
+# consistent with the DFMA micro-benchmark measured live below).  DESIGN.md "Roofline".
+FP64_LANES_PER_SM = 64
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def stop(self) -> dict:
+        self._stop.set()
+        self.join(timeout=6)
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg: int) -> str:
+    from workloads import CONFIG_NAMES
+    return CONFIG_NAMES[cfg]
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU legs: the oracle as it stands (oracle/sg_oracle.c, double build, OpenMP over targets)
+# --------------------------------------------------------------------------------------------------
+def oracle_sample_rate(lay, sigma, seconds: float, seed: int = 99):
+    """Time the oracle on a bounded, seeded sample of targets of this workload (every sampled target is
+    summed over ALL N leaves, so pairs/s does not depend on the sample size).  Returns
+    (pairs_per_s, threads, n_targets, elapsed_s)."""
+    import numpy as np
+    import oracle
+    from workloads import cell_rects, sample_targets
+    r = cell_rects(lay)
+    cores = os.cpu_count() or 1
+    n_cal = min(lay.n_cells, max(2 * cores, 8))
+    idx = sample_targets(lay, n_cal, seed)
+    t0 = time.perf_counter()
+    _, _, threads = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64")
+    dt = max(time.perf_counter() - t0, 1e-6)
+    rate = idx.size * lay.n_cells / dt
+    n = int(min(lay.n_cells, max(n_cal, seconds * rate / lay.n_cells)))
+    n = max(threads, (n // threads) * threads)
+    idx = sample_targets(lay, min(n, lay.n_cells), seed + 1)
+    t0 = time.perf_counter()
+    oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64")
+    dt = time.perf_counter() - t0
+    return idx.size * lay.n_cells / dt, threads, int(idx.size), dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores, same config / metric / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from workloads import make_config
+    lay, sigma = make_config(args.config)
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    rates, threads, n_t = [], 1, 0
+    for i in range(args.warmup + args.steps):
+        rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, per_step, seed=100 + i)
+        if i >= args.warmup:
+            rates.append((rate, dt))
+    total_pairs = sum(r * d for r, d in rates)
+    total_t = sum(d for _, d in rates)
+    value = total_pairs / total_t
+    sample = (f"{n_t} seeded targets per step (stratified by level), each summed over all "
+              f"{lay.n_cells} leaves, double-precision build of oracle/sg_oracle.c")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps),
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config), "n_cells": lay.n_cells,
+                   "pairs_per_evaluation": lay.n_cells ** 2},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+# the GPU path
+# --------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2001_02765_b200 import SgDisk, measure_fp64_peak, shard_range
+    from workloads import make_config, expected_counts
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    lay, sigma = make_config(args.config)
+    exp = expected_counts(args.config)
+    assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"], "frozen layout changed"
+    N = lay.n_cells
+    first, count = shard_range(N, rank, world)
+
+    d = SgDisk.from_layout(lay, device=local)
+    d.set_target_range(first, count)
+    info = d.layout_info()
+    model = d.kernel_model()
+    sd_launches, f_launches = d.launch_counts()
+
+    sigma_host = torch.from_numpy(np.ascontiguousarray(sigma)).pin_memory()
+    sigma_dev = sigma_host.to(dev)
+    Fx = torch.empty(count, dtype=torch.float64, device=dev)
+    Fy = torch.empty(count, dtype=torch.float64, device=dev)
+    Fx_host = torch.empty(count, dtype=torch.float64).pin_memory()
+    Fy_host = torch.empty(count, dtype=torch.float64).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step_resident():
+        flush.zero_()                       # L2 flush between steps (the vertex tiles are L2-sized)
+        d.set_density(sigma_dev)
+        d.force(Fx, Fy)
+
+    def step_e2e():
+        flush.zero_()
+        sigma_dev.copy_(sigma_host, non_blocking=True)
+        d.set_density(sigma_dev)
+        d.force(Fx, Fy)
+        Fx_host.copy_(Fx, non_blocking=True)
+        Fy_host.copy_(Fy, non_blocking=True)
+        torch.cuda.current_stream().synchronize()      # the caller holds the result on the host
+
+    peak_tflops, peak_winstr = measure_fp64_peak(local)
+
+    # ---- device-resident timing -------------------------------------------------------------------
+    for _ in range(max(3, args.warmup)):
+        step_resident()
+    d.set_kernel_timing(True)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step_resident()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    k_ms = d.kernel_times_ms()
+    d.set_kernel_timing(False)
+
+    # ---- end-to-end timing (host buffers, copies inside the timed region) --------------------------
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    t = torch.tensor([ms_total, e2e_s * 1e3, sum(k_ms) / max(1, len(k_ms))], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, e2e_ms, k_ms_avg = [float(v) for v in t.tolist()]
+
+    if rank == 0:
+        pairs = float(N) * float(N)
+        value = pairs * args.steps / (ms_total * 1e-3)
+        e2e_value = pairs * args.steps / (e2e_ms * 1e-3)
+        sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+        sm_max = clocks.get("sm_max_mhz") or 1965.0
+        nominal_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        evals = model["pair_evaluations"]                     # (targets of this rank) x N_v
+        achieved = evals * model["flops_per_pair"] / (k_ms_avg * 1e-3) / 1e12
+        winstr = evals * model["fp64_instr_per_pair"] / (k_ms_avg * 1e-3)
+        roofline = {
+            "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
+            "frac": achieved / nominal_tflops, "traffic": None,
+            "kernel": "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>",
+            "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / ms_total,
+            "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
+            "peak_measured_dfma_tflops": peak_tflops, "frac_of_measured_dfma": achieved / peak_tflops,
+            "fp64_pipe_util": winstr / (sm_count * FP64_LANES_PER_SM / 32.0 * sm_max * 1e6),
+            "fp64_pipe_util_of_measured_dfma": winstr / peak_winstr,
+            "flops_per_pair": model["flops_per_pair"], "fp64_instr_per_pair": model["fp64_instr_per_pair"],
+            "pair_evaluations_per_launch": evals,
+        }
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "n_cells": N, "n_vertices": info["n_vertices"],
+                       "pairs_per_evaluation": pairs, "parallelism": f"targets sharded over {world} GPU(s)",
+                       "l2": "256 MiB memset between steps (inside the timed region)"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 16 * count,
+                    "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": args.steps * (sd_launches + f_launches),
+            "clocks": clocks, "roofline": roofline,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds)
+            line["cpu_baseline"] = {
+                "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+                "sample": f"{n_t} seeded targets (stratified by level), each summed over all {N} leaves; "
+                          f"{dt:.1f} s; double-precision build of oracle/sg_oracle.c, OpenMP over targets"}
+        print(json.dumps(line), flush=True)
+    d.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

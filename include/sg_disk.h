@@ -109,11 +109,15 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 /* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
 int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
 
-/* Device time of the most recent sg_force interaction kernel launch is not recorded by the library;
- * callers time with their own events.  This diagnostic enqueues only the interaction kernel (S3)
- * on cuda_stream, between two events it owns, synchronises, and returns its duration in ms.  Used by
- * bench.py for the roofline line. */
-int sg_time_interaction_kernel(sg_ctx *ctx, void *cuda_stream, float *ms);
+/*
+ * Kernel timing for the roofline line.  While enabled, every sg_force records a pair of CUDA events
+ * on the caller's stream around the interaction kernel (S3) only; no synchronisation is added to
+ * sg_force.  sg_get_kernel_times synchronises on the newest end event and returns the durations (ms)
+ * of the sg_force calls made since timing was enabled, oldest first; at most 64 are kept.
+ *   ms: host [capacity];  n: host, receives the number written.
+ */
+int sg_set_kernel_timing(sg_ctx *ctx, int enable);
+int sg_get_kernel_times(sg_ctx *ctx, float *ms, int capacity, int *n);
 
 /* FP64-pipe instructions (warp-level, per (target, vertex) pair) and FP64 FLOPs per pair of the
  * interaction kernel as built (counted from its SASS); vertex evaluations per

@@ -20,7 +20,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 # every symbol include/sg_disk.h declares (tests check the header and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
-    "sg_set_density", "sg_force", "sg_set_target_range", "sg_launch_counts", "sg_time_interaction_kernel",
+    "sg_set_density", "sg_force", "sg_set_target_range", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
@@ -75,8 +75,10 @@ def load_library():
     lib.sg_set_target_range.argtypes = [vp, c_i64, c_i64]
     lib.sg_launch_counts.restype = c_int
     lib.sg_launch_counts.argtypes = [vp, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
-    lib.sg_time_interaction_kernel.restype = c_int
-    lib.sg_time_interaction_kernel.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_float)]
+    lib.sg_set_kernel_timing.restype = c_int
+    lib.sg_set_kernel_timing.argtypes = [vp, c_int]
+    lib.sg_get_kernel_times.restype = c_int
+    lib.sg_get_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), c_int, ctypes.POINTER(c_int)]
     lib.sg_kernel_model.restype = c_int
     lib.sg_kernel_model.argtypes = [vp, dp, dp, dp]
     lib.sg_measure_fp64_peak.restype = c_int
@@ -208,10 +210,14 @@ class SgDisk:
         self._check(self._lib.sg_launch_counts(self._ctx, ctypes.byref(a), ctypes.byref(b)))
         return a.value, b.value
 
-    def time_interaction_kernel(self) -> float:
-        ms = ctypes.c_float()
-        self._check(self._lib.sg_time_interaction_kernel(self._ctx, _stream_ptr(), ctypes.byref(ms)))
-        return float(ms.value)
+    def set_kernel_timing(self, enable: bool = True):
+        self._check(self._lib.sg_set_kernel_timing(self._ctx, int(bool(enable))))
+
+    def kernel_times_ms(self):
+        """Interaction-kernel durations (ms) of the force() calls since set_kernel_timing(True), oldest first."""
+        buf, n = (ctypes.c_float * 64)(), ctypes.c_int()
+        self._check(self._lib.sg_get_kernel_times(self._ctx, buf, 64, ctypes.byref(n)))
+        return [float(buf[i]) for i in range(n.value)]
 
     def kernel_model(self) -> dict:
         a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()

@@ -20,7 +20,13 @@ struct sg_ctx {
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
     std::string err;
+    // kernel timing ring (sg_set_kernel_timing)
+    bool timing = false;
+    int64_t timed_calls = 0;
+    std::vector<cudaEvent_t> ev0, ev1;
 };
+
+constexpr int kTimingRing = 64;
 
 static thread_local std::string g_create_error;
 
@@ -182,6 +188,8 @@ void sg_destroy(sg_ctx *c) {
         cudaSetDevice(c->device);
         cudaDeviceSynchronize();
         for (void *p : c->allocs) cudaFree(p);
+        for (cudaEvent_t e : c->ev0) cudaEventDestroy(e);
+        for (cudaEvent_t e : c->ev1) cudaEventDestroy(e);
     }
     delete c;
 }
@@ -235,7 +243,13 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     const ForcePlan p = make_plan(c);
     int rc = ensure_partials(c, p);
     if (rc) return rc;
+    const int slot = int(c->timed_calls % kTimingRing);
+    if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     launch_interaction(c->dev, p, s);
+    if (c->timing) {
+        SG_CUDA(c, cudaEventRecord(c->ev1[slot], s));
+        ++c->timed_calls;
+    }
     launch_finalise(c->dev, p, Fx_dev, Fy_dev, s);
     SG_CUDA(c, cudaGetLastError());
     return SG_OK;
@@ -257,25 +271,36 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
     return SG_OK;
 }
 
-int sg_time_interaction_kernel(sg_ctx *c, void *cuda_stream, float *ms) {
-    if (!c || !ms) return SG_ERR_ARG;
+int sg_set_kernel_timing(sg_ctx *c, int enable) {
+    if (!c) return SG_ERR_ARG;
     if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
-    if (!c->density_set) { c->err = "no density set"; return SG_ERR_STATE; }
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     SG_CUDA(c, cudaSetDevice(c->device));
-    const ForcePlan p = make_plan(c);
-    int rc = ensure_partials(c, p);
-    if (rc) return rc;
-    cudaEvent_t e0, e1;
-    SG_CUDA(c, cudaEventCreate(&e0));
-    SG_CUDA(c, cudaEventCreate(&e1));
-    SG_CUDA(c, cudaEventRecord(e0, s));
-    launch_interaction(c->dev, p, s);
-    SG_CUDA(c, cudaEventRecord(e1, s));
-    SG_CUDA(c, cudaEventSynchronize(e1));
-    SG_CUDA(c, cudaEventElapsedTime(ms, e0, e1));
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    SG_CUDA(c, cudaGetLastError());
+    if (enable && c->ev0.empty()) {
+        c->ev0.resize(kTimingRing); c->ev1.resize(kTimingRing);
+        for (int i = 0; i < kTimingRing; ++i) {
+            SG_CUDA(c, cudaEventCreate(&c->ev0[i]));
+            SG_CUDA(c, cudaEventCreate(&c->ev1[i]));
+        }
+    }
+    c->timing = enable != 0;
+    c->timed_calls = 0;
+    return SG_OK;
+}
+
+int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
+    if (!c || !ms || !n || capacity < 0) return SG_ERR_ARG;
+    *n = 0;
+    if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
+    const int64_t have = std::min<int64_t>(c->timed_calls, kTimingRing);
+    const int64_t take = std::min<int64_t>(have, capacity);
+    if (take == 0) return SG_OK;
+    SG_CUDA(c, cudaSetDevice(c->device));
+    SG_CUDA(c, cudaEventSynchronize(c->ev1[(c->timed_calls - 1) % kTimingRing]));
+    for (int64_t k = 0; k < take; ++k) {
+        const int slot = int((c->timed_calls - take + k) % kTimingRing);
+        SG_CUDA(c, cudaEventElapsedTime(&ms[k], c->ev0[slot], c->ev1[slot]));
+    }
+    *n = int(take);
     return SG_OK;
 }
 

@@ -62,6 +62,6 @@ cudaError_t measure_dfma(double *tflops, double *warp_instr_per_s);
 // FP64-pipe warp instructions and FLOPs per (target, vertex) pair of the interaction kernel as
 // written (cross-checked against cuobjdump -sass in DESIGN.md "Roofline").
 constexpr double kFp64InstrPerPair = 23.0;
-constexpr double kFlopsPerPair = 37.0;
+constexpr double kFlopsPerPair = 39.0;   // 16 DFMA x 2 + 4 DADD + 3 DMUL
 
 }  // namespace sg
