@@ -251,7 +251,7 @@ def run_ours(args):
         nominal_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         evals = model["pair_evaluations"]                     # (targets of this rank) x N_v
         achieved = evals * model["flops_per_pair"] / (k_ms_avg * 1e-3) / 1e12
-        winstr = evals * model["fp64_instr_per_pair"] / (k_ms_avg * 1e-3)
+        winstr = evals * model["fp64_instr_per_pair"] / 32.0 / (k_ms_avg * 1e-3)   # warp instructions / s
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
             "frac": achieved / nominal_tflops, "traffic": None,
