@@ -105,11 +105,7 @@ def measure_fp64_peak(device: int = 0):
     return tf.value, wi.value
 
 
-def shard_range(n: int, rank: int, world: int):
-    """Contiguous target slice [first, first+count) of rank ``rank`` out of ``world`` (sizes differ by <= 1)."""
-    base, rem = divmod(int(n), int(world))
-    first = rank * base + min(rank, rem)
-    return first, base + (1 if rank < rem else 0)
+from .sharding import shard_range  # noqa: E402,F401  (re-exported: one definition of the partition)
 
 
 def _stream_ptr():
