@@ -58,8 +58,8 @@ int upload(sg_ctx *c, T **p, const std::vector<T> &h) {
     return SG_OK;
 }
 
-// Work items = target blocks x source splits, walked round-robin by a persistent grid of
-// 2 CTAs per SM.  Pick the split count that keeps the last round of items fullest.
+// Work items = target blocks x source splits, pulled from an atomic queue by a persistent grid of
+// 2 CTAs per SM (about 16 items per CTA).  Pick the split count that keeps the last round fullest.
 ForcePlan make_plan(const sg_ctx *c) {
     ForcePlan p;
     p.first = c->first; p.count = c->count;
@@ -71,7 +71,7 @@ ForcePlan make_plan(const sg_ctx *c) {
     const int slots = c->sm_count * 2;
     const int n_tiles = c->dev.n_tiles;
     int best_split = 1; double best_eff = -1.0;
-    const int want = std::max(1, std::min(n_tiles, (4 * slots + p.n_tblocks - 1) / p.n_tblocks));
+    const int want = std::max(1, std::min(n_tiles, (16 * slots + p.n_tblocks - 1) / p.n_tblocks));
     for (int s = want; s <= std::min(n_tiles, want + 12); ++s) {
         const int tps = (n_tiles + s - 1) / s, ns = (n_tiles + tps - 1) / tps;
         const int64_t items = int64_t(ns) * p.n_tblocks;
@@ -109,7 +109,8 @@ int upload_layout(sg_ctx *c) {
     d.N = h.N; d.Nv = h.Nv;
     d.nX = int(h.colX.size()); d.nY = int(h.rowY.size());
     d.ntX = int(h.tX.size()); d.ntY = int(h.tY.size());
-    d.n_tiles = int((h.Nv + kTile - 1) / kTile);
+    d.n_tiles = int(h.chunk_x.size() / kChunksPerTile);
+    d.n_slots = int64_t(d.n_tiles) * kTileSlots;
     const int64_t tb_bytes = (int64_t(d.ntY) * d.nX + int64_t(d.ntX) * d.nY) * 8;
     if (tb_bytes > (int64_t(48) << 30)) {
         c->err = "line tables would need more than 48 GiB: layout too large for this build";
@@ -125,6 +126,9 @@ int upload_layout(sg_ctx *c) {
     if ((rc = upload(c, &d.colX, h.colX)) || (rc = upload(c, &d.colstart, h.colstart))) return rc;
     if ((rc = upload(c, &d.rowY, h.rowY)) || (rc = upload(c, &d.rowstart, h.rowstart))) return rc;
     if ((rc = upload(c, &d.rowperm, h.rowperm))) return rc;
+    if ((rc = upload(c, &d.chunk_x, h.chunk_x)) || (rc = upload(c, &d.slot_vertex, h.slot_vertex))) return rc;
+    if ((rc = dev_alloc(c, &d.queue, 1))) return rc;
+    SG_CUDA(c, cudaMemset(d.queue, 0, sizeof(unsigned int)));
     if ((rc = upload(c, &d.tX, h.tX)) || (rc = upload(c, &d.tY, h.tY))) return rc;
     if ((rc = dev_alloc(c, &d.vtile, int64_t(d.n_tiles) * kTileDoubles))) return rc;
     if ((rc = dev_alloc(c, &d.w, h.Nv))) return rc;
@@ -308,7 +312,7 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
     if (!c) return SG_ERR_ARG;
     if (fp64_instr_per_pair) *fp64_instr_per_pair = kFp64InstrPerPair;
     if (flops_per_pair) *flops_per_pair = kFlopsPerPair;
-    if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);
+    if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);   // algorithmic: real vertices
     return SG_OK;
 }
 

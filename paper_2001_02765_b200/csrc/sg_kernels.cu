@@ -86,16 +86,21 @@ void launch_build_logtab(const DevLayout &d, cudaStream_t s) {
 
 // ------------------------------------------------------------------------------------------------
 // S2a: vertex weights.  w_v = sum of +-sigma over the <= 4 cells that have v as a corner, in the fixed
-// order of the adjacency list (deterministic).  Writes the flat array and the w part of the tiles;
-// the padding slots of the last tile get w = 0.
+// order of the adjacency list (deterministic).  One thread per tile slot: writes the w half of the
+// slot's {y, w} pair (0 for padding slots) and the flat array used by the line tables.
 // ------------------------------------------------------------------------------------------------
-__global__ void vertex_weights_kernel(const int32_t *__restrict__ adj, const double *__restrict__ sigma,
-                                      double *__restrict__ w, double *__restrict__ vtile, int64_t Nv,
-                                      int64_t Nv_padded) {
-    const int64_t v = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (v >= Nv_padded) return;
+__device__ __forceinline__ double *slot_yw(double *vtile, int64_t slot) {
+    return vtile + (slot / kTileSlots) * kTileDoubles + kChunksPerTile + 2 * (slot % kTileSlots);
+}
+
+__global__ void vertex_weights_kernel(const int32_t *__restrict__ adj, const int32_t *__restrict__ slot_vertex,
+                                      const double *__restrict__ sigma, double *__restrict__ w,
+                                      double *__restrict__ vtile, int64_t n_slots) {
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= n_slots) return;
+    const int v = slot_vertex[s];
     double acc = 0.0;
-    if (v < Nv) {
+    if (v >= 0) {
         const int4 a = reinterpret_cast<const int4 *>(adj)[v];
         const int e[4] = {a.x, a.y, a.z, a.w};
 #pragma unroll
@@ -106,28 +111,37 @@ __global__ void vertex_weights_kernel(const int32_t *__restrict__ adj, const dou
             }
         w[v] = acc;
     }
-    vtile[(v / kTile) * kTileDoubles + 2 * kTile + (v % kTile)] = acc;
+    slot_yw(vtile, s)[1] = acc;
 }
 
 void launch_vertex_weights(const DevLayout &d, const double *sigma, cudaStream_t s) {
-    const int64_t padded = int64_t(d.n_tiles) * kTile;
-    vertex_weights_kernel<<<unsigned((padded + 255) / 256), 256, 0, s>>>(d.adj, sigma, d.w, d.vtile, d.Nv, padded);
+    vertex_weights_kernel<<<unsigned((d.n_slots + 255) / 256), 256, 0, s>>>(d.adj, d.slot_vertex, sigma, d.w, d.vtile,
+                                                                           d.n_slots);
 }
 
-// xy part of the tiles (lattice coordinates as FP64); padding = copy of vertex 0 (never on a target)
-__global__ void fill_static_tiles_kernel(const int32_t *__restrict__ vkx, const int32_t *__restrict__ vky,
-                                         double *__restrict__ vtile, int64_t Nv, int64_t Nv_padded) {
-    const int64_t v = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (v >= Nv_padded) return;
-    const int64_t src = v < Nv ? v : 0;
-    double2 *xy = reinterpret_cast<double2 *>(vtile + (v / kTile) * kTileDoubles);
-    xy[v % kTile] = make_double2(double(vkx[src]), double(vky[src]));
-    if (v >= Nv) vtile[(v / kTile) * kTileDoubles + 2 * kTile + (v % kTile)] = 0.0;
+// Static part of the tiles (lattice coordinates as FP64): xc per chunk, y per slot.  A padding slot takes
+// the y of its chunk's first vertex (of vertex 0 in an all-padding chunk, whose x is chunk 0's): a real
+// vertex position, so r > 0 against every target, and its w stays 0.
+__global__ void fill_static_tiles_kernel(const int32_t *__restrict__ vky, const int32_t *__restrict__ chunk_x,
+                                         const int32_t *__restrict__ slot_vertex, double *__restrict__ vtile,
+                                         int64_t n_slots) {
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= n_slots) return;
+    int v = slot_vertex[s];
+    if (v < 0) v = slot_vertex[(s / kChunk) * kChunk];
+    if (v < 0) v = 0;
+    double *yw = slot_yw(vtile, s);
+    yw[0] = double(vky[v]);
+    yw[1] = 0.0;
+    if (s % kChunk == 0) {
+        const int64_t c = s / kChunk;
+        vtile[(c / kChunksPerTile) * kTileDoubles + (c % kChunksPerTile)] = double(chunk_x[c]);
+    }
 }
 
 void launch_fill_static_tiles(const DevLayout &d, cudaStream_t s) {
-    const int64_t padded = int64_t(d.n_tiles) * kTile;
-    fill_static_tiles_kernel<<<unsigned((padded + 255) / 256), 256, 0, s>>>(d.vkx, d.vky, d.vtile, d.Nv, padded);
+    fill_static_tiles_kernel<<<unsigned((d.n_slots + 255) / 256), 256, 0, s>>>(d.vky, d.chunk_x, d.slot_vertex, d.vtile,
+                                                                              d.n_slots);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -166,22 +180,33 @@ void launch_line_tables(const DevLayout &d, cudaStream_t s) {
 // S3: the all-pairs interaction kernel.
 //
 // Work item = (target block of kThreads*T targets, source split of tiles_per_split vertex tiles).
-// A persistent grid walks the items round-robin (all items cost the same).  Per item each thread keeps
-// T targets and their two accumulators in registers; vertex tiles (24*kTile bytes: double2 xy[kTile],
-// double w[kTile]) arrive in shared memory through TMA bulk copies (cp.async.bulk + mbarrier
-// complete_tx), kStages deep; every thread reads every vertex of the tile as a warp-wide broadcast.
+// A persistent grid (2 CTAs per SM) pulls items from an atomic counter; every item writes its own slot of
+// `part`, so the result does not depend on which CTA ran it.  Per item each thread keeps T targets and
+// their accumulators in registers; vertex tiles (4,224 bytes: 16 chunk abscissae + 256 {y, w} slots)
+// arrive in shared memory through TMA bulk copies (cp.async.bulk + mbarrier complete_tx), kStages deep;
+// every thread reads every slot as a warp-wide broadcast.
 //
-// Per (target, vertex) pair, 23 FP64-pipe instructions, no branches, no division, no libdevice call:
-//   u, v, q = u^2+v^2                                   4   (exact: integers < 2^53)
+// A chunk is 16 vertices of one grid column, so u = xc - x_t, u^2 and the sign s(u) are shared by its
+// pairs: per (target, chunk) 2 DADD + 1 DMUL, and per (target, vertex) pair 21 FP64-pipe instructions,
+// no branch, no division, no libdevice call:
+//   v, q = v^2 + u^2                                    2   (exact: integers < 2^53)
 //   r = sqrt(q): MUFU.RSQ64H seed + one cubic step      5
 //   a1 = |v|+r, a2 = |u|+r                              2
-//   ln a_i = lntab[top bits of a_i] + log1p(a_i*c - 1)  2 x 5   (c = MUFU.RCP64H of the bin centre)
-//   accumulate +-w * ln a_i (sign by integer XOR)       2
+//   ln a_i = lntab[bin of a_i] + log1p(a_i*c - 1)       2 x 5   (c = MUFU.RCP64H of the bin centre)
+//   ax += w * s(v) ln a1 ;  cy += w * ln a2             2   (s(v) by integer XOR; s(u) once per chunk)
+// On sm_100 an FP64 instruction takes two issue cycles of a sub-partition and every other instruction
+// one (measured), so the non-FP64 instructions are kept few as well: the bin-centre
+// high word hc = (hi & keep) | half is both the MUFU.RCP64H operand and, shifted by 8, the table offset.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double fast_ln(double a, const double *tabp) {
+constexpr uint32_t kLogKeepMask = kLogKeep;
+
+// tabb = (const char*)stab - tab_idx0*8 - 4:  hc = idx << 11 | 0x400  =>  hc >> 8 = idx*8 + 4
+__device__ __forceinline__ double fast_ln(double a, const char *tabb, uint32_t keep) {
     const uint32_t hi = uint32_t(__double2hiint(a));
-    const double tv = tabp[hi >> kLogShift];
-    const double c = rcp_approx(__hiloint2double(int((hi & kLogKeep) | kLogHalfBin), 0));
+    uint32_t hc;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(hc) : "r"(hi), "r"(keep), "r"(kLogHalfBin));   // (hi & keep) | half
+    const double tv = *reinterpret_cast<const double *>(tabb + (hc >> 8));
+    const double c = rcp_approx(__hiloint2double(int(hc), 0));
     const double f = fma(a, c, -1.0);
     double s = fma(f, -0.25, 1.0 / 3.0);
     s = fma(f, s, -0.5);
@@ -189,8 +214,8 @@ __device__ __forceinline__ double fast_ln(double a, const double *tabp) {
     return fma(f, s, tv);
 }
 
-__device__ __forceinline__ double flip_sign_by(double w, double x) {   // w * s(x), s(+0) = +1
-    return __hiloint2double(__double2hiint(w) ^ (__double2hiint(x) & int(0x80000000u)), __double2loint(w));
+__device__ __forceinline__ double flip_sign_by(double a, double x) {   // a * s(x), s(+0) = +1
+    return __hiloint2double(__double2hiint(a) ^ (__double2hiint(x) & int(0x80000000u)), __double2loint(a));
 }
 
 template <int T>
@@ -198,11 +223,12 @@ __global__ void __launch_bounds__(kThreads, 2)
 interaction_kernel(const double2 *__restrict__ tgt, const double *__restrict__ vtile,
                    const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_tiles,
                    int tiles_per_split, int n_split, int n_tblocks, int64_t first, int64_t count,
-                   double *__restrict__ part) {
+                   double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *stile = reinterpret_cast<double *>(smem_raw);                         // kStages tiles
     uint64_t *full = reinterpret_cast<uint64_t *>(stile + kStages * kTileDoubles); // kStages mbarriers
     double *stab = reinterpret_cast<double *>(full + 8);                          // log table
+    __shared__ int s_item;
     const int tid = threadIdx.x;
 
     for (int i = tid; i < tab_entries; i += kThreads) stab[i] = lntab_g[i];
@@ -211,11 +237,15 @@ interaction_kernel(const double2 *__restrict__ tgt, const double *__restrict__ v
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    const double *tabp = stab - tab_idx0;
+    const char *tabb = reinterpret_cast<const char *>(stab) - int64_t(tab_idx0) * 8 - 4;
 
     uint32_t it = 0;   // tiles consumed by this CTA so far (stage = it % kStages, parity from it / kStages)
     const int n_items = n_tblocks * n_split;
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    while (true) {
+        if (tid == 0) s_item = int(atomicAdd(queue, 1u));
+        __syncthreads();
+        const int item = s_item;
+        if (item >= n_items) break;
         const int tb = item / n_split, sp = item - tb * n_split;
         const int tile0 = sp * tiles_per_split;
         const int ntile = min(tiles_per_split, n_tiles - tile0);
@@ -241,27 +271,34 @@ interaction_kernel(const double2 *__restrict__ tgt, const double *__restrict__ v
         for (int i = 0; i < ntile; ++i, ++it) {
             const uint32_t st = it % kStages;
             mbar_wait(&full[st], (it / kStages) & 1u);
-            const double2 *sxy = reinterpret_cast<const double2 *>(stile + st * kTileDoubles);
-            const double *sw = stile + st * kTileDoubles + 2 * kTile;
-#pragma unroll 2
-            for (int j = 0; j < kTile; ++j) {
-                const double2 xy = sxy[j];
-                const double w = sw[j];
+            const double *sx = stile + st * kTileDoubles;
+            const double2 *syw = reinterpret_cast<const double2 *>(sx + kChunksPerTile);
+#pragma unroll 1
+            for (int c = 0; c < kChunksPerTile; ++c) {
+                const double xc = sx[c];
+                double u[T], uu[T], cy[T];
 #pragma unroll
-                for (int k = 0; k < T; ++k) {
-                    const double u = xy.x - xt[k];
-                    const double v = xy.y - yt[k];
-                    const double q = fma(u, u, v * v);
-                    const double y0 = rsqrt_approx(q);
-                    const double t = q * y0;                 // ~sqrt(q)
-                    const double e = fma(-t, y0, 1.0);       // 1 - q*y0^2
-                    const double p = fma(0.375, e, 0.5);
-                    const double r = fma(t, p * e, t);       // t * (1 + e/2 + 3e^2/8)
-                    const double l1 = fast_ln(fabs(v) + r, tabp);
-                    const double l2 = fast_ln(fabs(u) + r, tabp);
-                    ax[k] = fma(flip_sign_by(w, v), l1, ax[k]);
-                    ay[k] = fma(flip_sign_by(w, u), l2, ay[k]);
+                for (int k = 0; k < T; ++k) { u[k] = xc - xt[k]; uu[k] = u[k] * u[k]; cy[k] = 0.0; }
+#pragma unroll 4
+                for (int j = 0; j < kChunk; ++j) {
+                    const double2 yw = syw[c * kChunk + j];
+#pragma unroll
+                    for (int k = 0; k < T; ++k) {
+                        const double v = yw.x - yt[k];
+                        const double q = fma(v, v, uu[k]);
+                        const double y0 = rsqrt_approx(q);
+                        const double t = q * y0;                 // ~sqrt(q)
+                        const double e = fma(-t, y0, 1.0);       // 1 - q*y0^2
+                        const double p = fma(0.375, e, 0.5);
+                        const double r = fma(t, p * e, t);       // t * (1 + e/2 + 3e^2/8)
+                        const double l1 = fast_ln(fabs(v) + r, tabb, keep);
+                        const double l2 = fast_ln(fabs(u[k]) + r, tabb, keep);
+                        ax[k] = fma(yw.y, flip_sign_by(l1, v), ax[k]);
+                        cy[k] = fma(yw.y, l2, cy[k]);
+                    }
                 }
+#pragma unroll
+                for (int k = 0; k < T; ++k) ay[k] += flip_sign_by(cy[k], u[k]);
             }
             __syncthreads();   // every thread is done with stage st
             if (tid == 0 && i + kStages < ntile) {
@@ -296,12 +333,12 @@ void launch_interaction(const DevLayout &d, const ForcePlan &p, cudaStream_t s) 
     if (p.count == 0) return;
     if (p.T == 4)
         interaction_kernel<4><<<p.grid, kThreads, p.smem, s>>>(d.tgt, d.vtile, d.lntab, d.tab_idx0, d.tab_entries,
-                                                              d.n_tiles, p.tiles_per_split, p.n_split,
-                                                              p.n_tblocks, p.first, p.count, d.part);
+                                                              d.n_tiles, p.tiles_per_split, p.n_split, p.n_tblocks,
+                                                              p.first, p.count, d.part, d.queue, kLogKeepMask);
     else
         interaction_kernel<1><<<p.grid, kThreads, p.smem, s>>>(d.tgt, d.vtile, d.lntab, d.tab_idx0, d.tab_entries,
-                                                              d.n_tiles, p.tiles_per_split, p.n_split,
-                                                              p.n_tblocks, p.first, p.count, d.part);
+                                                              d.n_tiles, p.tiles_per_split, p.n_split, p.n_tblocks,
+                                                              p.first, p.count, d.part, d.queue, kLogKeepMask);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -316,8 +353,10 @@ __global__ void finalise_kernel(const double2 *__restrict__ tgt, const int32_t *
                                 const int32_t *__restrict__ rowY, const double *__restrict__ TBx,
                                 const double *__restrict__ TBy, int nX, int nY,
                                 const double *__restrict__ part, int n_split, int64_t first, int64_t count,
-                                double G, double *__restrict__ Fx, double *__restrict__ Fy) {
+                                double G, double *__restrict__ Fx, double *__restrict__ Fy,
+                                unsigned int *__restrict__ queue) {
     const int64_t lt = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (lt == 0) *queue = 0u;   // the interaction kernel of this call has drained it; ready for the next call
     if (lt >= count) return;
     const int64_t t = first + lt;
     const double2 p = tgt[t];
@@ -347,7 +386,7 @@ void launch_finalise(const DevLayout &d, const ForcePlan &p, double *Fx, double 
     if (p.count == 0) return;
     finalise_kernel<<<unsigned((p.count + 127) / 128), 128, 0, s>>>(d.tgt, d.itx, d.ity, d.colX, d.rowY, d.TBx, d.TBy,
                                                                    d.nX, d.nY, d.part, p.n_split, p.first, p.count,
-                                                                   d.G, Fx, Fy);
+                                                                   d.G, Fx, Fy, d.queue);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -4,10 +4,15 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "sg_layout.h"
+
 namespace sg {
 
-constexpr int kTile = 256;            // vertices per shared-memory tile (one TMA bulk copy of 24*kTile B)
-constexpr int kTileDoubles = 3 * kTile;   // tile layout: double2 xy[kTile]; double w[kTile]
+// One shared-memory tile = kChunksPerTile chunks of kChunk vertices that share their x:
+//   double xc[kChunksPerTile];  double2 yw[kChunksPerTile * kChunk]  ( {y, w} per vertex slot )
+// = 4,224 bytes, moved by ONE TMA bulk copy.
+constexpr int kTileSlots = kChunksPerTile * kChunk;              // 256 vertex slots per tile
+constexpr int kTileDoubles = kChunksPerTile + 2 * kTileSlots;    // 528 doubles
 constexpr int kStages = 3;            // tiles in flight per CTA
 constexpr int kThreads = 256;         // threads per CTA of the interaction kernel
 constexpr int kLogK = 9;              // mantissa bits in the log-table index (|f| <= 2^-10 -> degree 4)
@@ -15,7 +20,8 @@ constexpr int kLogK = 9;              // mantissa bits in the log-table index (|
 struct DevLayout {
     int64_t N = 0, Nv = 0;
     int nX = 0, nY = 0, ntX = 0, ntY = 0;
-    int n_tiles = 0;                  // ceil(Nv / kTile)
+    int n_tiles = 0;                  // n_chunks / kChunksPerTile
+    int64_t n_slots = 0;              // n_tiles * kTileSlots (>= Nv: padding slots carry w = 0)
     double G = 1.0;
     // targets
     double2 *tgt = nullptr;           // [N] lattice (kx, ky) as FP64 (exact integers)
@@ -23,6 +29,8 @@ struct DevLayout {
     // vertices
     int32_t *adj = nullptr;           // [4 Nv]
     int32_t *vkx = nullptr, *vky = nullptr;   // [Nv]
+    int32_t *chunk_x = nullptr;       // [n_tiles * kChunksPerTile]
+    int32_t *slot_vertex = nullptr;   // [n_slots] vertex index or -1
     double *vtile = nullptr;          // [n_tiles * kTileDoubles]
     double *w = nullptr;              // [Nv]
     int32_t *colX = nullptr, *colstart = nullptr;           // [nX], [nX+1]
@@ -36,6 +44,7 @@ struct DevLayout {
     // split-source partial sums [n_split][2][count]
     double *part = nullptr;
     int64_t part_capacity = 0;        // doubles
+    unsigned int *queue = nullptr;    // work-item counter of the interaction kernel (reset by finalise)
 };
 
 struct ForcePlan {
@@ -44,7 +53,7 @@ struct ForcePlan {
     int tiles_per_split = 0;
     int64_t first = 0, count = 0;     // target range
     int n_tblocks = 0;                // ceil(count / (kThreads*T))
-    int grid = 0;                     // CTAs launched (persistent over work items)
+    int grid = 0;                     // CTAs launched (persistent, pull work items from the queue)
     size_t smem = 0;
 };
 
@@ -52,16 +61,17 @@ size_t interaction_smem_bytes(int tab_entries);
 cudaError_t configure_kernels(int tab_entries);   // cudaFuncSetAttribute for the opt-in smem size
 
 void launch_build_logtab(const DevLayout &d, cudaStream_t s);
-void launch_fill_static_tiles(const DevLayout &d, cudaStream_t s);        // xy part of vtile (once)
+void launch_fill_static_tiles(const DevLayout &d, cudaStream_t s);        // xc and y of vtile (once)
 void launch_vertex_weights(const DevLayout &d, const double *sigma, cudaStream_t s);
 void launch_line_tables(const DevLayout &d, cudaStream_t s);
 void launch_interaction(const DevLayout &d, const ForcePlan &p, cudaStream_t s);
 void launch_finalise(const DevLayout &d, const ForcePlan &p, double *Fx, double *Fy, cudaStream_t s);
 cudaError_t measure_dfma(double *tflops, double *warp_instr_per_s);
 
-// FP64-pipe warp instructions and FLOPs per (target, vertex) pair of the interaction kernel as
-// written (cross-checked against cuobjdump -sass in DESIGN.md "Roofline").
-constexpr double kFp64InstrPerPair = 23.0;
-constexpr double kFlopsPerPair = 39.0;   // 16 DFMA x 2 + 4 DADD + 3 DMUL
+// FP64-pipe warp instructions and FLOPs per (target, vertex slot) of the interaction kernel as written
+// (cross-checked against cuobjdump -sass): per pair 16 DFMA + 3 DADD + 2 DMUL,
+// plus per (target, chunk) 2 DADD + 1 DMUL shared by kChunk pairs.
+constexpr double kFp64InstrPerPair = 21.0 + 3.0 / kChunk;
+constexpr double kFlopsPerPair = 16 * 2 + 3 + 2 + 3.0 / kChunk;
 
 }  // namespace sg

@@ -177,6 +177,18 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     }
     L.rowstart.push_back(int32_t(L.Nv));
 
+    // chunks: cut every column into runs of kChunk vertices; pad the last run of a column with -1
+    for (size_t c = 0; c + 1 < L.colstart.size(); ++c)
+        for (int32_t s = L.colstart[c]; s < L.colstart[c + 1]; s += kChunk) {
+            L.chunk_x.push_back(L.colX[c]);
+            for (int j = 0; j < kChunk; ++j)
+                L.slot_vertex.push_back(s + j < L.colstart[c + 1] ? s + j : -1);
+        }
+    while (L.chunk_x.size() % kChunksPerTile) {          // whole tiles only
+        L.chunk_x.push_back(L.chunk_x[0]);
+        for (int j = 0; j < kChunk; ++j) L.slot_vertex.push_back(-1);
+    }
+
     // a target can never sit on a vertex (it is strictly inside its own leaf and leaves are disjoint):
     // cheap necessary check on the lattice -- both coordinates of a target being vertex coordinates is
     // only possible if some vertex lies inside a leaf, i.e. an overlap the patch test did not see.

@@ -34,7 +34,18 @@ struct HostLayout {
     std::vector<int32_t> colX, colstart;   // distinct vertex x (sorted); [nX+1]
     std::vector<int32_t> rowY, rowstart;   // distinct vertex y (sorted); [nY+1]
     std::vector<int32_t> rowperm;          // vertex indices sorted by (ky, kx)
+
+    // chunks: runs of <= kChunk consecutive vertices of ONE column (same x), so that u, u^2 and s(u)
+    // are shared by the whole chunk in the interaction kernel.  slot_vertex[c*kChunk + j] is the vertex
+    // in slot j of chunk c, or -1 for a padding slot (it gets w = 0 and the coordinates of the chunk's
+    // first vertex).  The chunk count is padded to a multiple of kChunksPerTile with copies of chunk 0
+    // whose slots are all -1.
+    std::vector<int32_t> chunk_x;          // [n_chunks]
+    std::vector<int32_t> slot_vertex;      // [n_chunks * kChunk]
 };
+
+constexpr int kChunk = 16;                 // vertices per chunk
+constexpr int kChunksPerTile = 16;         // chunks per shared-memory tile (one TMA bulk copy)
 
 // Returns SG_OK or SG_ERR_*; on error `err` holds the message.
 int build_layout(HostLayout &out, int n_levels, const double *cell_width, double x0, double y0,
