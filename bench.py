@@ -85,6 +85,19 @@ def parse_args():
     return ap.parse_args()
 
 
+def measured_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the interaction kernel from the committed ncu
+    capture of this workload (profiles/traffic.csv), or None if no capture exists for it."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(path):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return int(row["dram_bytes_per_launch"])
+    return None
+
+
 def workload_name(cfg: int) -> str:
     from workloads import CONFIG_NAMES
     return CONFIG_NAMES[cfg]
@@ -254,7 +267,8 @@ def run_ours(args):
         winstr = evals * model["fp64_instr_per_pair"] / 32.0 / (k_ms_avg * 1e-3)   # warp instructions / s
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
-            "frac": achieved / nominal_tflops, "traffic": None,
+            "frac": achieved / nominal_tflops,
+            "traffic": measured_traffic(workload_name(args.config)) if world == 1 else None,
             "kernel": "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>",
             "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / ms_total,
             "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
