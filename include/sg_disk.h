@@ -91,6 +91,18 @@ int sg_cell_geometry(const sg_ctx *ctx, double *xc, double *yc, double *h);
 int sg_set_density(sg_ctx *ctx, const double *sigma_dev, void *cuda_stream);
 
 /*
+ * S2 with the first-order Taylor terms of Eq. 6: on leaf c the density is
+ * sigma_c + dx_c (x - x_c) + dy_c (y - y_c), and the following sg_force calls sum
+ *     Fx_t = G * sum_c [ sigma_c K^{x,0} + dx_c K^{x,x} + dy_c K^{x,y} ]
+ * (same for y) -- the paper's second-order method.  sigma_dev, dx_dev, dy_dev: device [N], library cell
+ * order, FP64; slopes in physical units (d sigma / d x).  The paper does not say how slopes are obtained
+ * (its tables use the exact Taylor coefficients, R10): they are inputs here.  A later
+ * sg_set_density switches back to the zeroth-order sum.  Asynchronous on cuda_stream.
+ */
+int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx_dev, const double *dy_dev,
+                          void *cuda_stream);
+
+/*
  * S3-S5, the all-pairs sum.  Fx_dev, Fy_dev: device [N] (or [count] when a
  * target range is set, see below), FP64, written in library cell order.  Asynchronous on
  * cuda_stream.  Deterministic: the same context and sigma give bit-identical results run to run

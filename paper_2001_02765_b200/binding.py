@@ -20,7 +20,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 # every symbol include/sg_disk.h declares (tests check the header and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
-    "sg_set_density", "sg_force", "sg_set_target_range", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
+    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
@@ -69,6 +69,8 @@ def load_library():
     lib.sg_cell_geometry.argtypes = [vp, dp, dp, dp]
     lib.sg_set_density.restype = c_int
     lib.sg_set_density.argtypes = [vp, vp, vp]
+    lib.sg_set_density_linear.restype = c_int
+    lib.sg_set_density_linear.argtypes = [vp, vp, vp, vp, vp]
     lib.sg_force.restype = c_int
     lib.sg_force.argtypes = [vp, vp, vp, vp]
     lib.sg_set_target_range.restype = c_int
@@ -182,6 +184,15 @@ class SgDisk:
         """sigma: CUDA float64 tensor [N] in library cell order (asynchronous on the current stream)."""
         self._require_cuda(sigma, self.num_cells, "sigma")
         self._check(self._lib.sg_set_density(self._ctx, ctypes.c_void_p(sigma.data_ptr()), _stream_ptr()))
+
+    def set_density_linear(self, sigma, dx, dy):
+        """sigma, dx, dy: CUDA float64 tensors [N] (value and physical slopes of Eq. 6 per leaf); the next
+        force() calls include the slope terms."""
+        for t, name in ((sigma, "sigma"), (dx, "dx"), (dy, "dy")):
+            self._require_cuda(t, self.num_cells, name)
+        self._check(self._lib.sg_set_density_linear(self._ctx, ctypes.c_void_p(sigma.data_ptr()),
+                                                    ctypes.c_void_p(dx.data_ptr()), ctypes.c_void_p(dy.data_ptr()),
+                                                    _stream_ptr()))
 
     def set_target_range(self, first: int, count: int):
         self._check(self._lib.sg_set_target_range(self._ctx, int(first), int(count)))

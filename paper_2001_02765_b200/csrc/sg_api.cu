@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "sg_kernels.cuh"
+#include "sg_kernels_lin.cuh"
 #include "sg_layout.h"
 
 using namespace sg;
@@ -16,6 +17,8 @@ struct sg_ctx {
     int device = -1;             // < 0: host-only context (layout queries work, compute calls fail)
     int sm_count = 148;
     bool density_set = false;
+    bool linear = false;         // last density call carried slopes (sg_set_density_linear)
+    LinArrays lin;
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
@@ -63,9 +66,9 @@ int upload(sg_ctx *c, T **p, const std::vector<T> &h) {
 ForcePlan make_plan(const sg_ctx *c) {
     ForcePlan p;
     p.first = c->first; p.count = c->count;
-    p.smem = interaction_smem_bytes(c->dev.tab_entries);
+    p.smem = c->linear ? interaction_lin_smem_bytes(c->dev.tab_entries) : interaction_smem_bytes(c->dev.tab_entries);
     if (p.count == 0) return p;
-    p.T = p.count > 16384 ? 4 : 1;
+    p.T = c->linear ? lin_targets_per_thread() : (p.count > 16384 ? 4 : 1);
     const int64_t per_block = int64_t(kThreads) * p.T;
     p.n_tblocks = int((p.count + per_block - 1) / per_block);
     const int slots = c->sm_count * 2;
@@ -233,6 +236,38 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     launch_line_tables(c->dev, s);
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
+    c->linear = false;
+    return SG_OK;
+}
+
+int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_dev, const double *dy_dev,
+                          void *cuda_stream) {
+    if (!c) return SG_ERR_ARG;
+    if (!sigma_dev || !dx_dev || !dy_dev) { c->err = "sigma_dev / dx_dev / dy_dev is NULL"; return SG_ERR_ARG; }
+    if (c->device < 0) { c->err = "host-only context (device < 0): no CUDA path, and there is no CPU fallback"; return SG_ERR_CUDA; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    SG_CUDA(c, cudaSetDevice(c->device));
+    LinArrays &l = c->lin;
+    if (!l.allocated) {
+        const HostLayout &h = c->host;
+        const DevLayout &d = c->dev;
+        l.unit = h.unit;
+        l.cells_per_patch = h.P * h.P;
+        std::vector<double> hh(h.patches.size());
+        for (size_t p = 0; p < hh.size(); ++p) hh[p] = double(int64_t(1) << (h.n_levels - 1 - h.patches[p].level));
+        int rc;
+        if ((rc = upload(c, &l.patch_hh, hh))) return rc;
+        if ((rc = dev_alloc(c, &l.wl, 3 * h.Nv))) return rc;
+        if ((rc = dev_alloc(c, &l.vtile, int64_t(d.n_tiles) * kTileLinDoubles))) return rc;
+        if ((rc = dev_alloc(c, &l.TBx3, int64_t(d.ntY) * d.nX * 3))) return rc;
+        if ((rc = dev_alloc(c, &l.TBy3, int64_t(d.ntX) * d.nY * 3))) return rc;
+        SG_CUDA(c, configure_lin_kernels(d.tab_entries));
+        l.allocated = true;
+    }
+    launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
+    SG_CUDA(c, cudaGetLastError());
+    c->density_set = true;
+    c->linear = true;
     return SG_OK;
 }
 
@@ -249,12 +284,14 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (rc) return rc;
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
-    launch_interaction(c->dev, p, s);
+    if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
+    else launch_interaction(c->dev, p, s);
     if (c->timing) {
         SG_CUDA(c, cudaEventRecord(c->ev1[slot], s));
         ++c->timed_calls;
     }
-    launch_finalise(c->dev, p, Fx_dev, Fy_dev, s);
+    if (c->linear) launch_finalise_lin(c->dev, c->lin, p, Fx_dev, Fy_dev, s);
+    else launch_finalise(c->dev, p, Fx_dev, Fy_dev, s);
     SG_CUDA(c, cudaGetLastError());
     return SG_OK;
 }
@@ -310,8 +347,8 @@ int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
 
 int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_per_pair, double *pair_evaluations) {
     if (!c) return SG_ERR_ARG;
-    if (fp64_instr_per_pair) *fp64_instr_per_pair = kFp64InstrPerPair;
-    if (flops_per_pair) *flops_per_pair = kFlopsPerPair;
+    if (fp64_instr_per_pair) *fp64_instr_per_pair = c->linear ? kLinFp64InstrPerPair : kFp64InstrPerPair;
+    if (flops_per_pair) *flops_per_pair = c->linear ? kLinFlopsPerPair : kFlopsPerPair;
     if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);   // algorithmic: real vertices
     return SG_OK;
 }

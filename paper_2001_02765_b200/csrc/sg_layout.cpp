@@ -44,7 +44,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
         }
     }
     const int64_t N = n_patches * int64_t(P) * P;
-    if (N >= (int64_t(1) << 30)) { err = "too many cells (limit 2^30)"; return SG_ERR_LAYOUT; }
+    if (N >= (int64_t(1) << 29)) { err = "too many cells (limit 2^29)"; return SG_ERR_LAYOUT; }
 
     L = HostLayout();
     L.n_levels = n_levels; L.P = P; L.x0 = x0; L.y0 = y0; L.N = N;
@@ -148,8 +148,8 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
         for (size_t k = 0; k < 4; ++k) {
             if (r + k < e) {
                 const uint32_t cc = rec[r + k].cc;
-                const uint32_t corner = cc & 3u, neg = (corner == 1u || corner == 2u) ? 1u : 0u;
-                L.adj.push_back(int32_t(((cc >> 2) << 1) | neg));
+                // (cell << 2) | corner; corner 0 = NE (+), 1 = NW (-), 2 = SE (-), 3 = SW (+)
+                L.adj.push_back(int32_t(cc));
             } else {
                 L.adj.push_back(-1);
             }

@@ -30,7 +30,7 @@ struct HostLayout {
     // vertices (deduplicated cell corners), sorted by (kx, ky): column c is the contiguous range
     // [colstart[c], colstart[c+1]) and is sorted by ky inside.
     std::vector<int32_t> vkx, vky;
-    std::vector<int32_t> adj;              // [4*Nv]: (cell << 1) | neg, or -1; neg=1 for NW / SE corners
+    std::vector<int32_t> adj;              // [4*Nv]: (cell << 2) | corner, or -1; corner 0 NE(+) 1 NW(-) 2 SE(-) 3 SW(+)
     std::vector<int32_t> colX, colstart;   // distinct vertex x (sorted); [nX+1]
     std::vector<int32_t> rowY, rowstart;   // distinct vertex y (sorted); [nY+1]
     std::vector<int32_t> rowperm;          // vertex indices sorted by (ky, kx)
