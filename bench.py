@@ -82,6 +82,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slopes", action="store_true",
+                    help="time the first-order path (sg_set_density_linear); default is the zeroth-order hot path")
     return ap.parse_args()
 
 
@@ -195,11 +197,25 @@ def run_ours(args):
     d = SgDisk.from_layout(lay, device=local)
     d.set_target_range(first, count)
     info = d.layout_info()
-    model = d.kernel_model()
     sd_launches, f_launches = d.launch_counts()
 
-    sigma_host = torch.from_numpy(np.ascontiguousarray(sigma)).pin_memory()
-    sigma_dev = sigma_host.to(dev)
+    fields = [sigma]
+    if args.slopes:
+        # first-order Taylor coefficients of the smooth Kuzmin profile every bench config is
+        # built on (cfg 3/4: centred differences of the cell samples along the library's own rows would need the
+        # neighbour links; analytic slopes of the base profile are the paper's choice, R10)
+        from workloads.configs import cell_centres
+        xc, yc, _ = cell_centres(lay)
+        g = -3.0 * sigma / (xc * xc + yc * yc + 0.04)
+        fields += [g * xc, g * yc]
+    hosts = [torch.from_numpy(np.ascontiguousarray(f)).pin_memory() for f in fields]
+    devs = [h.to(dev) for h in hosts]
+
+    def set_density():
+        if args.slopes:
+            d.set_density_linear(*devs)
+        else:
+            d.set_density(devs[0])
     Fx = torch.empty(count, dtype=torch.float64, device=dev)
     Fy = torch.empty(count, dtype=torch.float64, device=dev)
     Fx_host = torch.empty(count, dtype=torch.float64).pin_memory()
@@ -208,13 +224,14 @@ def run_ours(args):
 
     def step_resident():
         flush.zero_()                       # L2 flush between steps (the vertex tiles are L2-sized)
-        d.set_density(sigma_dev)
+        set_density()
         d.force(Fx, Fy)
 
     def step_e2e():
         flush.zero_()
-        sigma_dev.copy_(sigma_host, non_blocking=True)
-        d.set_density(sigma_dev)
+        for dv, h in zip(devs, hosts):
+            dv.copy_(h, non_blocking=True)
+        set_density()
         d.force(Fx, Fy)
         Fx_host.copy_(Fx, non_blocking=True)
         Fy_host.copy_(Fy, non_blocking=True)
@@ -225,6 +242,7 @@ def run_ours(args):
     # ---- device-resident timing -------------------------------------------------------------------
     for _ in range(max(3, args.warmup)):
         step_resident()
+    model = d.kernel_model()                # of the path the warm-up just selected (zeroth order / slopes)
     d.set_kernel_timing(True)
     sampler = ClockSampler(local)
     barrier()
@@ -268,8 +286,9 @@ def run_ours(args):
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
             "frac": achieved / nominal_tflops,
-            "traffic": measured_traffic(workload_name(args.config)) if world == 1 else None,
-            "kernel": "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>",
+            "traffic": measured_traffic(workload_name(args.config)) if world == 1 and not args.slopes else None,
+            "kernel": ("interaction_lin_kernel<4>" if args.slopes else
+                       "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"),
             "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / ms_total,
             "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
             "peak_measured_dfma_tflops": peak_tflops, "frac_of_measured_dfma": achieved / peak_tflops,
@@ -283,9 +302,11 @@ def run_ours(args):
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config), "n_cells": N, "n_vertices": info["n_vertices"],
-                       "pairs_per_evaluation": pairs, "parallelism": f"targets sharded over {world} GPU(s)",
+                       "pairs_per_evaluation": pairs,
+                       "order": "sigma0 + slope terms (Eq. 6)" if args.slopes else "sigma0 (north_star hot path)",
+                       "parallelism": f"targets sharded over {world} GPU(s)",
                        "l2": "256 MiB memset between steps (inside the timed region)"},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 16 * count,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N * len(fields), "d2h_bytes_per_step": 16 * count,
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": args.steps * (sd_launches + f_launches),
             "clocks": clocks, "roofline": roofline,

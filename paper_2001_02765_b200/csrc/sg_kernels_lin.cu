@@ -106,7 +106,7 @@ void launch_weights_lin(const DevLayout &d, const LinArrays &l, const double *si
 // The partial sums hold the main parts of F/G directly:
 //   x:  -Wt s(v) L1 + a v s(u) L2 - c r        y:  -Wt s(u) L2 + c u s(v) L1 - a r
 // ------------------------------------------------------------------------------------------------
-constexpr int kLinT = 2;
+constexpr int kLinT = 4;
 int lin_targets_per_thread() { return kLinT; }
 
 template <int T>
