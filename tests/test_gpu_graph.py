@@ -1,0 +1,43 @@
+"""a time-stepping caller (1e4 steps) can capture sg_set_density + sg_force in a
+CUDA graph: after one warm-up call the library enqueues only kernel launches on the caller's stream (no
+allocation, no synchronisation), so the pair is capturable and replays with new sigma contents."""
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+def test_step_is_cuda_graph_capturable():
+    import torch
+    from paper_2001_02765_b200 import SgDisk
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required")
+    lay, sigma = make_config(2)
+    rng = np.random.default_rng(0)
+    sig_a = torch.as_tensor(sigma).cuda()
+    sig_b = torch.as_tensor(sigma * (1.0 + 0.1 * rng.uniform(-1, 1, sigma.size))).cuda()
+    with SgDisk.from_layout(lay, device=0) as d:
+        buf = sig_a.clone()
+        Fx = torch.empty(lay.n_cells, dtype=torch.float64, device="cuda")
+        Fy = torch.empty_like(Fx)
+        d.set_density(buf); d.force(Fx, Fy)                 # warm-up: sizes the partial-sum buffer
+        torch.cuda.synchronize()
+        ref_a = (Fx.clone(), Fy.clone())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            d.set_density(buf)
+            d.force(Fx, Fy)
+        buf.copy_(sig_b)
+        g.replay()
+        torch.cuda.synchronize()
+        got_b = (Fx.clone(), Fy.clone())
+        d.set_density(sig_b); eager = d.force()
+        torch.cuda.synchronize()
+        assert torch.equal(got_b[0], eager[0]) and torch.equal(got_b[1], eager[1])      # deterministic: bit-equal
+        buf.copy_(sig_a)
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(Fx, ref_a[0]) and torch.equal(Fy, ref_a[1])
+        assert not torch.equal(ref_a[0], got_b[0])
