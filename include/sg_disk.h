@@ -118,6 +118,18 @@ int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
  */
 int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 
+/*
+ * How sg_force evaluates the O(N^2) interaction sum (S3) of the zeroth-order path.
+ *   SG_MODE_DIRECT   every (target, vertex) pair: 1 sqrt + 2 ln (the north_star kernel; always available; default)
+ *   SG_MODE_LATTICE  lattice-offset reuse: per (target patch, source patch) the pair function
+ *                    is tabulated once on the patch pair's offset lattice and the pairs reduce to 2 FMA each;
+ *                    patch pairs more than one level apart are summed directly.  Needs P = 8 or 16
+ *                    (SG_ERR_ARG otherwise).  Same sum, same tolerances; the slope path always runs DIRECT.
+ */
+#define SG_MODE_DIRECT  0
+#define SG_MODE_LATTICE 1
+int sg_set_interaction_mode(sg_ctx *ctx, int mode);
+
 /* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
 int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
 

@@ -20,7 +20,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 # every symbol include/sg_disk.h declares (tests check the header and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
-    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
+    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
@@ -75,6 +75,8 @@ def load_library():
     lib.sg_force.argtypes = [vp, vp, vp, vp]
     lib.sg_set_target_range.restype = c_int
     lib.sg_set_target_range.argtypes = [vp, c_i64, c_i64]
+    lib.sg_set_interaction_mode.restype = c_int
+    lib.sg_set_interaction_mode.argtypes = [vp, c_int]
     lib.sg_launch_counts.restype = c_int
     lib.sg_launch_counts.argtypes = [vp, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
     lib.sg_set_kernel_timing.restype = c_int
@@ -197,6 +199,10 @@ class SgDisk:
     def set_target_range(self, first: int, count: int):
         self._check(self._lib.sg_set_target_range(self._ctx, int(first), int(count)))
         self._first, self._count = int(first), int(count)
+
+    def set_interaction_mode(self, mode: str):
+        """'direct' (every pair: sqrt + 2 ln) or 'lattice' (per-patch-pair offset tables; P = 8 or 16)."""
+        self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1}[mode]))
 
     def force(self, Fx=None, Fy=None):
         """Fx, Fy (CUDA float64 [count]) at the leaf centres of the current target range."""

@@ -7,6 +7,7 @@
 
 #include "sg_kernels.cuh"
 #include "sg_kernels_lin.cuh"
+#include "sg_kernels_patch.cuh"
 #include "sg_layout.h"
 
 using namespace sg;
@@ -19,6 +20,8 @@ struct sg_ctx {
     bool density_set = false;
     bool linear = false;         // last density call carried slopes (sg_set_density_linear)
     LinArrays lin;
+    PatchArrays patch;           // lattice-offset reuse path (P = 8 or 16)
+    bool use_patch = false;      // sg_set_interaction_mode
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
@@ -106,6 +109,44 @@ int ensure_partials(sg_ctx *c, const ForcePlan &p) {
     return SG_OK;
 }
 
+// Lattice-offset path: one work item = (target patch, split of the source patch list).
+PatchPlan make_patch_plan(const sg_ctx *c) {
+    PatchPlan pp;
+    const PatchArrays &pa = c->patch;
+    const int64_t PP = int64_t(pa.P) * pa.P;
+    pp.smem = patch_smem_bytes(pa.P, c->dev.tab_entries);
+    if (c->count == 0) return pp;
+    pp.first_patch = int(c->first / PP);
+    pp.n_tpatches = int((c->first + c->count - 1) / PP) - pp.first_patch + 1;
+    const int slots = c->sm_count * (pa.P == 16 ? 2 : 4);
+    int want = (8 * slots + pp.n_tpatches - 1) / pp.n_tpatches;            // about 8 items per resident CTA
+    want = std::max(1, std::min(want, std::max(1, pa.n_patches / 4)));     // but >= 4 source patches per item
+    pp.patches_per_split = (pa.n_patches + want - 1) / want;
+    pp.n_split = (pa.n_patches + pp.patches_per_split - 1) / pp.patches_per_split;
+    pp.grid = int(std::min<int64_t>(int64_t(pp.n_split) * pp.n_tpatches, slots));
+    return pp;
+}
+
+int upload_patches(sg_ctx *c) {
+    const HostLayout &h = c->host;
+    PatchArrays &pa = c->patch;
+    if (h.P != 8 && h.P != 16) return SG_OK;                               // direct kernel only
+    pa.P = h.P;
+    pa.n_patches = int(h.patches.size());
+    pa.wstride = ((h.P + 1) * (h.P + 1) + 1) & ~1;
+    std::vector<PatchInfo> info(h.patches.size());
+    for (size_t p = 0; p < info.size(); ++p) {
+        const int32_t cw = int32_t(2) << (h.n_levels - 1 - h.patches[p].level);
+        info[p] = PatchInfo{h.patches[p].i0 * cw, h.patches[p].j0 * cw, cw, h.patches[p].level};
+    }
+    int rc;
+    if ((rc = upload(c, &pa.info, info))) return rc;
+    if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
+    SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
+    pa.enabled = true;
+    return SG_OK;
+}
+
 int upload_layout(sg_ctx *c) {
     const HostLayout &h = c->host;
     DevLayout &d = c->dev;
@@ -151,6 +192,7 @@ int upload_layout(sg_ctx *c) {
     launch_fill_static_tiles(d, nullptr);
     SG_CUDA(c, cudaGetLastError());
     SG_CUDA(c, cudaDeviceSynchronize());
+    if ((rc = upload_patches(c))) return rc;
     return SG_OK;
 }
 
@@ -234,6 +276,7 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     SG_CUDA(c, cudaSetDevice(c->device));
     launch_vertex_weights(c->dev, sigma_dev, s);
     launch_line_tables(c->dev, s);
+    if (c->patch.enabled) launch_patch_weights(c->patch, sigma_dev, s);
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = false;
@@ -279,12 +322,19 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (!Fx_dev || !Fy_dev) { c->err = "Fx_dev / Fy_dev is NULL"; return SG_ERR_ARG; }
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     SG_CUDA(c, cudaSetDevice(c->device));
-    const ForcePlan p = make_plan(c);
+    ForcePlan p = make_plan(c);
+    const bool by_patch = c->use_patch && !c->linear;
+    PatchPlan pp;
+    if (by_patch) {
+        pp = make_patch_plan(c);
+        p.n_split = pp.n_split;            // finalise adds pp.n_split partial sums per target
+    }
     int rc = ensure_partials(c, p);
     if (rc) return rc;
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
+    else if (by_patch) launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, s);
     else launch_interaction(c->dev, p, s);
     if (c->timing) {
         SG_CUDA(c, cudaEventRecord(c->ev1[slot], s));
@@ -293,6 +343,16 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (c->linear) launch_finalise_lin(c->dev, c->lin, p, Fx_dev, Fy_dev, s);
     else launch_finalise(c->dev, p, Fx_dev, Fy_dev, s);
     SG_CUDA(c, cudaGetLastError());
+    return SG_OK;
+}
+
+int sg_set_interaction_mode(sg_ctx *c, int mode) {
+    if (!c) return SG_ERR_ARG;
+    if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE) { c->err = "unknown interaction mode"; return SG_ERR_ARG; }
+    if (mode == SG_MODE_LATTICE && c->host.P != 8 && c->host.P != 16) {
+        c->err = "SG_MODE_LATTICE needs patches of 8 x 8 or 16 x 16 cells"; return SG_ERR_ARG;
+    }
+    c->use_patch = mode == SG_MODE_LATTICE;
     return SG_OK;
 }
 
@@ -307,7 +367,8 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
 
 int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     if (!c) return SG_ERR_ARG;
-    if (set_density_launches) *set_density_launches = 3;      // vertex weights, column table, row table
+    // vertex weights, column table, row table (+ per-patch weights when the lattice-offset path exists)
+    if (set_density_launches) *set_density_launches = 3 + ((c->patch.enabled && !c->linear) ? 1 : 0);
     if (force_launches) *force_launches = c->count > 0 ? 2 : 0;   // interaction, finalise
     return SG_OK;
 }

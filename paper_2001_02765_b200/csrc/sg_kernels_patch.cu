@@ -1,0 +1,158 @@
+// sg_kernels_patch.cu -- S3 by lattice-offset reuse.
+//
+// The interaction sum M^x_t = sum_v w_v s(v) ln(|v|+r), M^y_t = sum_v w_v s(u) ln(|u|+r) (sg_kernels.cu header) is
+// evaluated patch against patch.  For a target patch A (P x P cell centres, pitch cw_A) and a source patch B
+// ((P+1)^2 vertices, pitch cw_B) every offset is
+//     u = u00 + g (i rb - k ra),   v = v00 + g (j rb - l ra),     g = min(cw_A, cw_B), ra = cw_A/g, rb = cw_B/g,
+// so only M^2 distinct (u, v) occur, M = P rb + (P-1) ra + 1, for P^2 (P+1)^2 pairs.  The CTA tabulates
+//     T[n][m] = { s(v) ln(|v|+r), s(u) ln(|u|+r) }
+// once per patch pair in shared memory (same sqrt / table-driven log as the direct kernel) and the pair sum becomes
+// a correlation with the patch's own signed vertex weights w^B (cells of B only; the weights of all patches at a
+// shared vertex add up to the deduplicated w_v, so the sum over patches is the same sum):
+//     M^x[l][k] += sum_{j,i} w^B[j][i] T[j rb - l ra][i rb - k ra].x          (2 DFMA per pair)
+// Patch pairs more than one level apart (large M) are summed directly, pair by pair, in the same kernel.
+// The separable ln|u| part, the coincidence rule and the epilogue are unchanged (finalise_kernel).
+#include "sg_device.cuh"
+#include "sg_kernels_patch.cuh"
+
+namespace sg {
+
+constexpr int kPatchMaxM = 48;        // table path for |level difference| <= 1: M <= 3P <= 48
+
+// per-patch signed vertex weights: vertex (i,j) of patch p is the NE corner of its cell (i-1,j-1) (+), the NW
+// corner of (i,j-1) (-), the SE corner of (i-1,j) (-) and the SW corner of (i,j) (+)   [[.]] of PAPER.md:92
+__global__ void patch_weights_kernel(const double *__restrict__ sigma, double *__restrict__ wP, int P, int wstride,
+                                     int n_patches) {
+    const int p = blockIdx.x;
+    const double *s = sigma + int64_t(p) * P * P;
+    for (int e = threadIdx.x; e < wstride; e += blockDim.x) {
+        double w = 0.0;
+        if (e < (P + 1) * (P + 1)) {
+            const int i = e % (P + 1), j = e / (P + 1);
+            if (i >= 1 && j >= 1) w += s[(j - 1) * P + (i - 1)];
+            if (i < P && j >= 1) w -= s[(j - 1) * P + i];
+            if (i >= 1 && j < P) w -= s[j * P + (i - 1)];
+            if (i < P && j < P) w += s[j * P + i];
+        }
+        wP[int64_t(p) * wstride + e] = w;
+    }
+}
+
+void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s) {
+    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, pa.wP, pa.P, pa.wstride, pa.n_patches);
+}
+
+__device__ __forceinline__ double2 pair_terms(double u, double v, const char *tabb, uint32_t keep) {
+    const double q = fma(u, u, v * v);
+    const double y0 = rsqrt_approx(q);
+    const double t = q * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double r = fma(t, p * e, t);
+    return make_double2(flip_sign_by(fast_ln(fabs(v) + r, tabb, keep), v),
+                        flip_sign_by(fast_ln(fabs(u) + r, tabb, keep), u));
+}
+
+template <int P>
+__global__ void __launch_bounds__(P * P, (P == 16 ? 2 : 4))
+patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ wP, int wstride,
+                         const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_patches,
+                         int patches_per_split, int n_split, int first_patch, int n_tpatches, int64_t first,
+                         int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
+    constexpr int NT = P * P, NV = (P + 1) * (P + 1);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2 *stab2 = reinterpret_cast<double2 *>(smem_raw);                        // kPatchMaxM^2 pair table
+    double *sw = reinterpret_cast<double *>(stab2 + kPatchMaxM * kPatchMaxM);     // weights of B
+    double *stab = sw + ((NV + 1) & ~1);                                          // log table
+    __shared__ int s_item;
+    const int tid = threadIdx.x, k = tid % P, l = tid / P;
+
+    for (int i = tid; i < tab_entries; i += NT) stab[i] = lntab_g[i];
+    __syncthreads();
+    const char *tabb = reinterpret_cast<const char *>(stab) - int64_t(tab_idx0) * 8 - 4;
+
+    const int n_items = n_tpatches * n_split;
+    while (true) {
+        if (tid == 0) s_item = int(atomicAdd(queue, 1u));
+        __syncthreads();
+        const int item = s_item;
+        if (item >= n_items) break;
+        const int ta = item / n_split, sp = item - ta * n_split;
+        const PatchInfo A = info[first_patch + ta];
+        const int b0 = sp * patches_per_split, b1 = min(n_patches, b0 + patches_per_split);
+        const int xt = A.X0 + k * A.cw + A.cw / 2, yt = A.Y0 + l * A.cw + A.cw / 2;     // lattice, exact
+        double ax = 0.0, ay = 0.0;
+
+        for (int b = b0; b < b1; ++b) {
+            const PatchInfo B = info[b];
+            __syncthreads();                                   // previous pair is done with sw / stab2
+            for (int e = tid; e < NV; e += NT) sw[e] = wP[int64_t(b) * wstride + e];
+            const int dl = A.level - B.level;
+            if (dl >= -1 && dl <= 1) {
+                const int g = min(A.cw, B.cw), ra = A.cw / g, rb = B.cw / g;
+                const int M = P * rb + (P - 1) * ra + 1, mmin = (P - 1) * ra;
+                const int u00 = B.X0 - (A.X0 + A.cw / 2), v00 = B.Y0 - (A.Y0 + A.cw / 2);
+                for (int e = tid; e < M * M; e += NT) {
+                    const int mm = e % M, nn = e / M;
+                    stab2[e] = pair_terms(double(u00 + (mm - mmin) * g), double(v00 + (nn - mmin) * g), tabb, keep);
+                }
+                __syncthreads();
+                const double2 *trow = stab2 + ((P - 1 - l) * ra) * M + (P - 1 - k) * ra;
+                const double *wrow = sw;
+                for (int j = 0; j <= P; ++j, trow += rb * M, wrow += P + 1) {
+#pragma unroll
+                    for (int i = 0; i <= P; ++i) {
+                        const double2 T = trow[i * rb];
+                        const double w = wrow[i];
+                        ax = fma(w, T.x, ax);
+                        ay = fma(w, T.y, ay);
+                    }
+                }
+            } else {
+                __syncthreads();
+                const double *wrow = sw;
+                for (int j = 0; j <= P; ++j, wrow += P + 1) {
+                    const double v = double(B.Y0 + j * B.cw - yt);
+#pragma unroll 2
+                    for (int i = 0; i <= P; ++i) {
+                        const double2 T = pair_terms(double(B.X0 + i * B.cw - xt), v, tabb, keep);
+                        ax = fma(wrow[i], T.x, ax);
+                        ay = fma(wrow[i], T.y, ay);
+                    }
+                }
+            }
+        }
+        const int64_t lt = (int64_t(first_patch + ta) * NT + tid) - first;      // local index in the target range
+        if (lt >= 0 && lt < count) {
+            part[(int64_t(sp) * 2 + 0) * count + lt] = ax;
+            part[(int64_t(sp) * 2 + 1) * count + lt] = ay;
+        }
+    }
+}
+
+size_t patch_smem_bytes(int P, int tab_entries) {
+    const int NV = (P + 1) * (P + 1);
+    return size_t(kPatchMaxM) * kPatchMaxM * 16 + size_t((NV + 1) & ~1) * 8 + size_t(tab_entries) * 8;
+}
+
+cudaError_t configure_patch_kernels(int P, int tab_entries) {
+    const int bytes = int(patch_smem_bytes(P, tab_entries));
+    if (P == 16)
+        return cudaFuncSetAttribute(patch_interaction_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return cudaFuncSetAttribute(patch_interaction_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
+                              int64_t count, cudaStream_t s) {
+    if (count == 0) return;
+    if (pa.P == 16)
+        patch_interaction_kernel<16><<<pp.grid, 256, pp.smem, s>>>(
+            pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue, kLogKeepMask);
+    else
+        patch_interaction_kernel<8><<<pp.grid, 64, pp.smem, s>>>(
+            pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue, kLogKeepMask);
+}
+
+}  // namespace sg
