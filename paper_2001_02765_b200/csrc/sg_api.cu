@@ -127,6 +127,21 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
     return pp;
 }
 
+// Blocked same-level kernel: one work item = (group of 8 target patches, split of the source patch list).
+PatchPlan make_blocked_plan(const sg_ctx *c) {
+    PatchPlan pb = make_patch_plan(c);
+    pb.smem = patch_blocked_smem_bytes(c->dev.tab_entries);
+    if (c->count == 0) return pb;
+    const int n_groups = (pb.n_tpatches + 7) / 8, slots = c->sm_count;
+    const int n_patches = c->patch.n_patches;
+    int want = (8 * slots + n_groups - 1) / n_groups;
+    want = std::max(1, std::min(want, std::max(1, n_patches / 8)));
+    pb.patches_per_split = (n_patches + want - 1) / want;
+    pb.n_split = (n_patches + pb.patches_per_split - 1) / pb.patches_per_split;
+    pb.grid = int(std::min<int64_t>(int64_t(pb.n_split) * n_groups, slots));
+    return pb;
+}
+
 int upload_patches(sg_ctx *c) {
     const HostLayout &h = c->host;
     PatchArrays &pa = c->patch;
@@ -143,6 +158,10 @@ int upload_patches(sg_ctx *c) {
     if ((rc = upload(c, &pa.info, info))) return rc;
     if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
     SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
+    if (pa.P == 16 && patch_blocked_smem_bytes(c->dev.tab_entries) <= size_t(227) * 1024) {
+        SG_CUDA(c, configure_patch_blocked(c->dev.tab_entries));
+        pa.blocked = true;
+    }
     pa.enabled = true;
     return SG_OK;
 }
@@ -171,8 +190,8 @@ int upload_layout(sg_ctx *c) {
     if ((rc = upload(c, &d.rowY, h.rowY)) || (rc = upload(c, &d.rowstart, h.rowstart))) return rc;
     if ((rc = upload(c, &d.rowperm, h.rowperm))) return rc;
     if ((rc = upload(c, &d.chunk_x, h.chunk_x)) || (rc = upload(c, &d.slot_vertex, h.slot_vertex))) return rc;
-    if ((rc = dev_alloc(c, &d.queue, 1))) return rc;
-    SG_CUDA(c, cudaMemset(d.queue, 0, sizeof(unsigned int)));
+    if ((rc = dev_alloc(c, &d.queue, 2))) return rc;
+    SG_CUDA(c, cudaMemset(d.queue, 0, 2 * sizeof(unsigned int)));
     if ((rc = upload(c, &d.tX, h.tX)) || (rc = upload(c, &d.tY, h.tY))) return rc;
     if ((rc = dev_alloc(c, &d.vtile, int64_t(d.n_tiles) * kTileDoubles))) return rc;
     if ((rc = dev_alloc(c, &d.w, h.Nv))) return rc;
@@ -324,17 +343,30 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     SG_CUDA(c, cudaSetDevice(c->device));
     ForcePlan p = make_plan(c);
     const bool by_patch = c->use_patch && !c->linear;
-    PatchPlan pp;
+    PatchPlan pp, pb;                      // cross-level / generic kernel, blocked same-level kernel
+    bool blocked = false, cross = true;
     if (by_patch) {
         pp = make_patch_plan(c);
-        p.n_split = pp.n_split;            // finalise adds pp.n_split partial sums per target
+        blocked = c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count;   // small problems: more, lighter CTAs
+        if (blocked) {
+            pb = make_blocked_plan(c);
+            cross = c->host.n_levels > 1;
+            p.n_split = pb.n_split + (cross ? pp.n_split : 0);
+        } else {
+            p.n_split = pp.n_split;        // finalise adds p.n_split partial sums per target
+        }
     }
     int rc = ensure_partials(c, p);
     if (rc) return rc;
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
-    else if (by_patch) launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, s);
+    else if (by_patch) {
+        if (blocked) launch_patch_same_level(c->dev, c->patch, pb, c->first, c->count, s);
+        if (cross) launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count,
+                                            c->dev.part + (blocked ? int64_t(pb.n_split) * 2 * c->count : 0),
+                                            blocked ? 1 : 0, s);
+    }
     else launch_interaction(c->dev, p, s);
     if (c->timing) {
         SG_CUDA(c, cudaEventRecord(c->ev1[slot], s));

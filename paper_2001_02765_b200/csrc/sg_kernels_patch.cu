@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(P * P, (P == 16 ? 2 : 4))
 patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ wP, int wstride,
                          const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_patches,
                          int patches_per_split, int n_split, int first_patch, int n_tpatches, int64_t first,
-                         int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
+                         int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep,
+                         int skip_same_level) {
     constexpr int NT = P * P, NV = (P + 1) * (P + 1);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2 *stab2 = reinterpret_cast<double2 *>(smem_raw);                        // kPatchMaxM^2 pair table
@@ -85,6 +86,7 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 
         for (int b = b0; b < b1; ++b) {
             const PatchInfo B = info[b];
+            if (skip_same_level && B.level == A.level) continue;   // done by patch_same_level_kernel (CTA-uniform)
             __syncthreads();                                   // previous pair is done with sw / stab2
             for (int e = tid; e < NV; e += NT) sw[e] = wP[int64_t(b) * wstride + e];
             const int dl = A.level - B.level;
@@ -130,6 +132,119 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Same-level patch pairs, P = 16, register-blocked: ONE WARP per target patch, 8 targets per thread
+// (lane = l + 16 kb owns row l, columns 8 kb .. 8 kb + 7), private offset table and weight buffer per warp, no
+// CTA-wide barrier in the pair loop.  With ra = rb = 1 the table column of (vertex i, target k) is i - k + 15, so
+// one loaded T[row][cc] serves the 8 targets of a thread against 8 consecutive vertices: per table load 16 DFMA,
+// the vertex weights slide through an 8-deep register window (w rows are zero-padded by 7 on the left and 8 on the
+// right, which also takes care of the ragged ends).  Table rows are 33 entries apart so that the 8 lanes of an
+// LDS.128 quarter-warp (8 consecutive l = 8 consecutive table rows) hit 8 different 16-byte bank groups.
+// ------------------------------------------------------------------------------------------------
+constexpr int kBlkWarps = 8, kBlkR = 8, kBlkTRow = 33, kBlkT = 32 * kBlkTRow, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
+
+__global__ void __launch_bounds__(kBlkWarps * 32, 1)
+patch_same_level_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ wP, int wstride,
+                        const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_patches,
+                        int patches_per_split, int n_split, int first_patch, int n_tpatches, int64_t first,
+                        int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
+    constexpr int P = 16;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                                // [warp][32][33]
+    double *sW = reinterpret_cast<double *>(sT + kBlkWarps * kBlkT);                    // [warp][17][32]
+    double *stab = sW + kBlkWarps * kBlkW;                                              // log table
+    __shared__ int s_item;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int l = lane & 15, k0 = (lane >> 4) * kBlkR;
+
+    for (int i = tid; i < tab_entries; i += kBlkWarps * 32) stab[i] = lntab_g[i];
+    for (int i = tid; i < kBlkWarps * kBlkW; i += kBlkWarps * 32) sW[i] = 0.0;          // zero padding stays zero
+    __syncthreads();
+    const char *tabb = reinterpret_cast<const char *>(stab) - int64_t(tab_idx0) * 8 - 4;
+    double2 *T = sT + warp * kBlkT;
+    double *W = sW + warp * kBlkW;
+
+    const int n_groups = (n_tpatches + kBlkWarps - 1) / kBlkWarps;
+    const int n_items = n_groups * n_split;
+    while (true) {
+        __syncthreads();
+        if (tid == 0) s_item = int(atomicAdd(queue, 1u));
+        __syncthreads();
+        const int item = s_item;
+        if (item >= n_items) break;
+        const int grp = item / n_split, sp = item - grp * n_split;
+        const int ta = grp * kBlkWarps + warp;
+        if (ta >= n_tpatches) continue;                        // whole warp: nothing to do in this group
+        const PatchInfo A = info[first_patch + ta];
+        const int b0 = sp * patches_per_split, b1 = min(n_patches, b0 + patches_per_split);
+        double ax[kBlkR], ay[kBlkR];
+#pragma unroll
+        for (int r = 0; r < kBlkR; ++r) { ax[r] = 0.0; ay[r] = 0.0; }
+
+        for (int b = b0; b < b1; ++b) {
+            const PatchInfo B = info[b];
+            if (B.level != A.level) continue;                  // other levels: patch_interaction_kernel
+            __syncwarp();
+            for (int e = lane; e < (P + 1) * (P + 1); e += 32) {
+                const int i = e % (P + 1), j = e / (P + 1);
+                W[j * kBlkWRow + 7 + i] = wP[int64_t(b) * wstride + e];
+            }
+            const int g = A.cw, u00 = B.X0 - (A.X0 + g / 2), v00 = B.Y0 - (A.Y0 + g / 2);
+#pragma unroll 4
+            for (int e = lane; e < 32 * 32; e += 32) {
+                const int mm = e & 31, nn = e >> 5;
+                T[nn * kBlkTRow + mm] = pair_terms(double(u00 + (mm - 15) * g), double(v00 + (nn - 15) * g), tabb, keep);
+            }
+            __syncwarp();
+            const int cbase = 8 - k0;
+            for (int j = 0; j <= P; ++j) {
+                const double2 *trow = T + (j - l + 15) * kBlkTRow + cbase;
+                const double *wrow = W + j * kBlkWRow;
+                double win[8];
+#pragma unroll
+                for (int r = 0; r < 7; ++r) win[r] = wrow[r];
+#pragma unroll
+                for (int t = 0; t < P + kBlkR; ++t) {
+                    win[(t + 7) & 7] = wrow[t + 7];
+                    const double2 Tv = trow[t];
+#pragma unroll
+                    for (int r = 0; r < kBlkR; ++r) {
+                        if (t + r >= 7 && t + r <= 7 + P) {      // vertex i = t + r - 7 exists (compile-time)
+                            ax[r] = fma(win[(t + r) & 7], Tv.x, ax[r]);
+                            ay[r] = fma(win[(t + r) & 7], Tv.y, ay[r]);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < kBlkR; ++r) {
+            const int64_t lt = (int64_t(first_patch + ta) * (P * P) + l * P + k0 + r) - first;
+            if (lt >= 0 && lt < count) {
+                part[(int64_t(sp) * 2 + 0) * count + lt] = ax[r];
+                part[(int64_t(sp) * 2 + 1) * count + lt] = ay[r];
+            }
+        }
+    }
+}
+
+size_t patch_blocked_smem_bytes(int tab_entries) {
+    return size_t(kBlkWarps) * (kBlkT * 16 + kBlkW * 8) + size_t(tab_entries) * 8;
+}
+
+cudaError_t configure_patch_blocked(int tab_entries) {
+    return cudaFuncSetAttribute(patch_same_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(patch_blocked_smem_bytes(tab_entries)));
+}
+
+void launch_patch_same_level(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
+                             int64_t count, cudaStream_t s) {
+    if (count == 0) return;
+    patch_same_level_kernel<<<pp.grid, kBlkWarps * 32, pp.smem, s>>>(
+        pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split, pp.n_split,
+        pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue + 1, kLogKeepMask);
+}
+
 size_t patch_smem_bytes(int P, int tab_entries) {
     const int NV = (P + 1) * (P + 1);
     return size_t(kPatchMaxM) * kPatchMaxM * 16 + size_t((NV + 1) & ~1) * 8 + size_t(tab_entries) * 8;
@@ -143,16 +258,16 @@ cudaError_t configure_patch_kernels(int P, int tab_entries) {
 }
 
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                              int64_t count, cudaStream_t s) {
+                              int64_t count, double *part, int skip_same_level, cudaStream_t s) {
     if (count == 0) return;
     if (pa.P == 16)
         patch_interaction_kernel<16><<<pp.grid, 256, pp.smem, s>>>(
             pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
-            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue, kLogKeepMask);
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_same_level);
     else
         patch_interaction_kernel<8><<<pp.grid, 64, pp.smem, s>>>(
             pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
-            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue, kLogKeepMask);
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_same_level);
 }
 
 }  // namespace sg

@@ -12,6 +12,7 @@ struct PatchInfo {                    // one leaf patch on the integer lattice
 
 struct PatchArrays {
     bool enabled = false;             // P is 8 or 16
+    bool blocked = false;             // P == 16 and the per-warp tables + log table fit in shared memory
     int P = 0;
     int n_patches = 0;
     int wstride = 0;                  // doubles per patch in wP: (P+1)^2 rounded up to a multiple of 2
@@ -30,6 +31,11 @@ size_t patch_smem_bytes(int P, int tab_entries);
 cudaError_t configure_patch_kernels(int P, int tab_entries);
 void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s);
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                              int64_t count, cudaStream_t s);
+                              int64_t count, double *part, int skip_same_level, cudaStream_t s);
+// register-blocked same-level kernel (P = 16); uses the second queue counter (d.queue + 1), writes d.part slots
+size_t patch_blocked_smem_bytes(int tab_entries);
+cudaError_t configure_patch_blocked(int tab_entries);
+void launch_patch_same_level(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
+                             int64_t count, cudaStream_t s);
 
 }  // namespace sg
