@@ -1,0 +1,112 @@
+"""GPU parity of the lattice-offset reuse path (SG_MODE_LATTICE) against the CPU oracle, at the
+same north_star tolerances as the direct kernel, on all five BASELINE.json configs, plus its edge cases."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import Layout, make_config, cell_rects, sample_targets, paper_ilr_layout, nested_layout, kuzmin_sigma
+from workloads.configs import cell_centres
+
+pytestmark = pytest.mark.gpu
+TOL_MAX, TOL_L2 = 1e-11, 1e-12
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+def gpu_force(torch, lay, sigma, mode="lattice", target_range=None):
+    from paper_2001_02765_b200 import SgDisk
+    with SgDisk.from_layout(lay, device=0) as d:
+        d.set_interaction_mode(mode)
+        d.set_density(torch.as_tensor(sigma, dtype=torch.float64).cuda())
+        if target_range is not None:
+            d.set_target_range(*target_range)
+        Fx, Fy = d.force()
+        torch.cuda.synchronize()
+        return Fx.cpu().numpy(), Fy.cpu().numpy()
+
+
+def check(gx, gy, ox, oy):
+    assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
+    scale = max(np.abs(ox).max(), np.abs(oy).max())
+    emax = max(np.abs(gx - ox).max(), np.abs(gy - oy).max()) / scale
+    l2 = np.sqrt((np.sum((gx - ox) ** 2) + np.sum((gy - oy) ** 2)) / (np.sum(ox ** 2) + np.sum(oy ** 2)))
+    assert emax <= TOL_MAX and l2 <= TOL_L2, (emax, l2)
+
+
+def oracle_force(lay, sigma, idx):
+    r = cell_rects(lay)
+    fx, fy, _ = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f80")
+    return fx, fy
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_small_configs_all_targets(torch_cuda, cfg):
+    """cfg 1: P = 16, one level (generic kernel, too small for the blocked one); cfg 2: P = 8, two levels."""
+    lay, sigma = make_config(cfg)
+    gx, gy = gpu_force(torch_cuda, lay, sigma)
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+
+
+@pytest.mark.parametrize("cfg,seed", [(3, 2003), (4, 2004), (5, 2007)])
+def test_large_configs_sampled_targets(torch_cuda, cfg, seed):
+    """cfg 3: four levels (pairs up to three levels apart: table path and in-kernel direct path); cfg 4: three
+    levels, blocked same-level kernel + cross-level kernel; cfg 5: one level, blocked kernel only."""
+    lay, sigma = make_config(cfg)
+    gx, gy = gpu_force(torch_cuda, lay, sigma)
+    cores = os.cpu_count() or 1
+    n = int(min(4096, max(256, 1.0e8 * min(cores, 64) / lay.n_cells / 4)))
+    idx = sample_targets(lay, n, seed)
+    ox, oy = oracle_force(lay, sigma, idx)
+    check(gx[idx], gy[idx], ox, oy)
+    assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
+
+
+def test_modes_agree_and_are_deterministic(torch_cuda):
+    lay, sigma = make_config(4)
+    a = gpu_force(torch_cuda, lay, sigma, "lattice")
+    b = gpu_force(torch_cuda, lay, sigma, "lattice")
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])          # bit-identical run to run
+    c = gpu_force(torch_cuda, lay, sigma, "direct")
+    s = max(np.abs(c[0]).max(), np.abs(c[1]).max())
+    assert max(np.abs(a[0] - c[0]).max(), np.abs(a[1] - c[1]).max()) <= 1e-12 * s
+
+
+def test_target_range_slices(torch_cuda):
+    """Ranges that start and end inside patches (the kernels work on whole target patches and mask the stores)."""
+    lay, sigma = make_config(4)
+    fx, fy = gpu_force(torch_cuda, lay, sigma)
+    n = lay.n_cells
+    s = max(np.abs(fx).max(), np.abs(fy).max())
+    for first, count in ((0, 1), (100, 300000), (300100, n - 300100), (n - 1, 1), (255, 2), (17, 0)):
+        gx, gy = gpu_force(torch_cuda, lay, sigma, target_range=(first, count))
+        assert gx.shape == (count,)
+        if count:
+            assert np.abs(gx - fx[first:first + count]).max() <= 1e-13 * s
+            assert np.abs(gy - fy[first:first + count]).max() <= 1e-13 * s
+
+
+def test_five_nested_levels_small_patches(torch_cuda):
+    """P = 8, five levels: every kind of patch pair (same level, one level apart both ways, farther apart)."""
+    lay = nested_layout(5, 32, 8.0, 8)
+    x, y, _ = cell_centres(lay)
+    sigma = kuzmin_sigma(x, y, a=0.3) * (1 + 0.2 * np.random.default_rng(12).uniform(-1, 1, lay.n_cells))
+    gx, gy = gpu_force(torch_cuda, lay, sigma)
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+
+
+def test_unsupported_patch_size_is_refused(torch_cuda):
+    from paper_2001_02765_b200 import SgDisk, SgError, binding
+    lay = paper_ilr_layout(32, 2)                                  # P = 1 quadtree
+    with SgDisk.from_layout(lay, device=0) as d:
+        with pytest.raises(SgError) as e:
+            d.set_interaction_mode("lattice")
+        assert e.value.code == binding.SG_ERR_ARG
+        d.set_interaction_mode("direct")
