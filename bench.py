@@ -82,6 +82,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="auto", choices=["auto", "direct", "lattice"],
+                    help="S3 algorithm: direct pair sum, lattice-offset reuse, or auto (lattice when the layout allows)")
     ap.add_argument("--slopes", action="store_true",
                     help="time the first-order path (sg_set_density_linear); default is the zeroth-order hot path")
     return ap.parse_args()
@@ -197,7 +199,6 @@ def run_ours(args):
     d = SgDisk.from_layout(lay, device=local)
     d.set_target_range(first, count)
     info = d.layout_info()
-    sd_launches, f_launches = d.launch_counts()
 
     fields = [sigma]
     if args.slopes:
@@ -240,23 +241,41 @@ def run_ours(args):
     peak_tflops, peak_winstr = measure_fp64_peak(local)
 
     # ---- device-resident timing -------------------------------------------------------------------
-    for _ in range(max(3, args.warmup)):
+    def timed_resident(steps, warmup):
+        """W warm-up steps, then `steps` steps between CUDA events with a barrier + synchronize on both sides; the
+        interaction kernel(s) of every step are timed by the library's own event ring on the same stream."""
+        for _ in range(warmup):
+            step_resident()
+        mdl = d.kernel_model()              # of the path the warm-up just selected
+        d.set_kernel_timing(True)
+        smp = ClockSampler(local)
+        barrier()
+        smp.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            step_resident()
+        e1.record()
+        barrier()
+        clk = smp.stop()
+        total = e0.elapsed_time(e1)
+        kms = d.kernel_times_ms()
+        d.set_kernel_timing(False)
+        return total, kms, clk, mdl
+
+    lattice = (not args.slopes) and args.mode != "direct" and lay.P in (8, 16)
+    if args.mode == "lattice" and not lattice:
+        raise SystemExit("--mode lattice needs the zeroth-order path and 8x8 or 16x16 patches")
+    d.set_interaction_mode("lattice" if lattice else "direct")
+    sd_launches, f_launches = d.launch_counts()
+    ms_total, k_ms, clocks, model = timed_resident(args.steps, max(3, args.warmup))
+    direct_run = None
+    if lattice and world == 1:
+        # the north_star kernel (every pair: sqrt + 2 ln) on the same workload, same run, for its roofline line
+        d.set_interaction_mode("direct")
+        direct_run = timed_resident(2, 1)
+        d.set_interaction_mode("lattice")
         step_resident()
-    model = d.kernel_model()                # of the path the warm-up just selected (zeroth order / slopes)
-    d.set_kernel_timing(True)
-    sampler = ClockSampler(local)
-    barrier()
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step_resident()
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    k_ms = d.kernel_times_ms()
-    d.set_kernel_timing(False)
 
     # ---- end-to-end timing (host buffers, copies inside the timed region) --------------------------
     for _ in range(2):
@@ -280,23 +299,31 @@ def run_ours(args):
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         nominal_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-        evals = model["pair_evaluations"]                     # (targets of this rank) x N_v
-        achieved = evals * model["flops_per_pair"] / (k_ms_avg * 1e-3) / 1e12
-        winstr = evals * model["fp64_instr_per_pair"] / 32.0 / (k_ms_avg * 1e-3)   # warp instructions / s
-        roofline = {
-            "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
-            "frac": achieved / nominal_tflops,
-            "traffic": measured_traffic(workload_name(args.config)) if world == 1 and not args.slopes else None,
-            "kernel": ("interaction_lin_kernel<4>" if args.slopes else
-                       "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"),
-            "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / ms_total,
-            "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
-            "peak_measured_dfma_tflops": peak_tflops, "frac_of_measured_dfma": achieved / peak_tflops,
-            "fp64_pipe_util": winstr / (sm_count * FP64_LANES_PER_SM / 32.0 * sm_max * 1e6),
-            "fp64_pipe_util_of_measured_dfma": winstr / peak_winstr,
-            "flops_per_pair": model["flops_per_pair"], "fp64_instr_per_pair": model["fp64_instr_per_pair"],
-            "pair_evaluations_per_launch": evals,
-        }
+        def roofline_of(mdl, kms, step_ms, kernel, traffic):
+            evals = mdl["pair_evaluations"]                   # algorithmic units one launch processes
+            achieved = evals * mdl["flops_per_pair"] / (kms * 1e-3) / 1e12
+            winstr = evals * mdl["fp64_instr_per_pair"] / 32.0 / (kms * 1e-3)      # warp instructions / s
+            return {
+                "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
+                "frac": achieved / nominal_tflops, "traffic": traffic, "kernel": kernel,
+                "kernel_ms": kms, "kernel_share_of_step": kms / step_ms,
+                "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
+                "peak_measured_dfma_tflops": peak_tflops, "frac_of_measured_dfma": achieved / peak_tflops,
+                "fp64_pipe_util": winstr / (sm_count * FP64_LANES_PER_SM / 32.0 * sm_max * 1e6),
+                "fp64_pipe_util_of_measured_dfma": winstr / peak_winstr,
+                "flops_per_pair": mdl["flops_per_pair"], "fp64_instr_per_pair": mdl["fp64_instr_per_pair"],
+                "pair_evaluations_per_launch": evals,
+            }
+
+        direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
+        direct_traffic = measured_traffic(workload_name(args.config)) if world == 1 else None
+        if args.slopes:
+            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>", None)
+        elif lattice:
+            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps,
+                                   "patch_same_level_kernel (+ patch_interaction_kernel on multi-level layouts)", None)
+        else:
+            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, direct_name, direct_traffic)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -304,6 +331,7 @@ def run_ours(args):
             "config": {"workload": workload_name(args.config), "n_cells": N, "n_vertices": info["n_vertices"],
                        "pairs_per_evaluation": pairs,
                        "order": "sigma0 + slope terms (Eq. 6)" if args.slopes else "sigma0 (north_star hot path)",
+                       "interaction_mode": "lattice-offset reuse (SG_MODE_LATTICE)" if lattice else "direct",
                        "parallelism": f"targets sharded over {world} GPU(s)",
                        "l2": "256 MiB memset between steps (inside the timed region)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N * len(fields), "d2h_bytes_per_step": 16 * count,
@@ -311,6 +339,14 @@ def run_ours(args):
             "gpu_launches": args.steps * (sd_launches + f_launches),
             "clocks": clocks, "roofline": roofline,
         }
+        if direct_run is not None:
+            d_total, d_kms, _, d_model = direct_run
+            d_k = sum(d_kms) / max(1, len(d_kms))
+            line["direct_kernel"] = {
+                "what": "same workload, same run, SG_MODE_DIRECT: every (target, vertex) pair = 1 sqrt + 2 ln "
+                        "(the north_star interaction kernel); 2 timed steps after 1 warm-up",
+                "value": pairs * 2 / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / 2,
+                "roofline": roofline_of(d_model, d_k, d_total / 2, direct_name, direct_traffic)}
         if not args.no_cpu_baseline and world == 1:
             rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds)
             line["cpu_baseline"] = {

@@ -401,7 +401,14 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
     if (!c) return SG_ERR_ARG;
     // vertex weights, column table, row table (+ per-patch weights when the lattice-offset path exists)
     if (set_density_launches) *set_density_launches = 3 + ((c->patch.enabled && !c->linear) ? 1 : 0);
-    if (force_launches) *force_launches = c->count > 0 ? 2 : 0;   // interaction, finalise
+    if (force_launches) {                                         // interaction kernel(s) + finalise
+        int n = 1;
+        if (c->use_patch && !c->linear && c->count > 0) {
+            const PatchPlan pp = make_patch_plan(c);
+            if (c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count && c->host.n_levels > 1) n = 2;
+        }
+        *force_launches = c->count > 0 ? n + 1 : 0;
+    }
     return SG_OK;
 }
 
@@ -440,6 +447,15 @@ int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
 
 int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_per_pair, double *pair_evaluations) {
     if (!c) return SG_ERR_ARG;
+    if (c->use_patch && !c->linear) {
+        // lattice-offset path: one pair = (target, per-patch vertex) = 2 DFMA of the correlation; the offset tables
+        // ((2P)^2 pair-function evaluations per P^2 (P+1)^2 pairs, 1.4 % at P = 16) are not credited
+        const double nsrc = double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
+        if (fp64_instr_per_pair) *fp64_instr_per_pair = 2.0;
+        if (flops_per_pair) *flops_per_pair = 4.0;
+        if (pair_evaluations) *pair_evaluations = double(c->count) * nsrc;
+        return SG_OK;
+    }
     if (fp64_instr_per_pair) *fp64_instr_per_pair = c->linear ? kLinFp64InstrPerPair : kFp64InstrPerPair;
     if (flops_per_pair) *flops_per_pair = c->linear ? kLinFlopsPerPair : kFlopsPerPair;
     if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);   // algorithmic: real vertices
