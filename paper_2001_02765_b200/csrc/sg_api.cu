@@ -207,7 +207,10 @@ int upload_layout(sg_ctx *c) {
     d.tab_entries = (e_max + 1) << kLogK;
     if ((rc = dev_alloc(c, &d.lntab, d.tab_entries))) return rc;
     SG_CUDA(c, configure_kernels(d.tab_entries));
+    d.lnint_n = h.extent < (1 << 21) ? h.extent + 2 : 0;        // all |vertex - target| lattice distances
+    if (d.lnint_n > 0 && (rc = dev_alloc(c, &d.lnint, d.lnint_n))) return rc;
     launch_build_logtab(d, nullptr);
+    launch_build_lnint(d, nullptr);
     launch_fill_static_tiles(d, nullptr);
     SG_CUDA(c, cudaGetLastError());
     SG_CUDA(c, cudaDeviceSynchronize());

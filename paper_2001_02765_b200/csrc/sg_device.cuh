@@ -82,4 +82,11 @@ __device__ __forceinline__ double flip_sign_by(double a, double x) {   // a * s(
     return __hiloint2double(__double2hiint(a) ^ (__double2hiint(x) & int(0x80000000u)), __double2loint(a));
 }
 
+// ln|d| of an integer lattice distance; 0 for d == 0 (the coincident grid line is skipped)
+__device__ __forceinline__ double ln_lattice(int d, const double *__restrict__ lnint, int lnint_n) {
+    const int a = abs(d);
+    if (lnint_n > 0) return lnint[a];
+    return a ? log(double(a)) : 0.0;
+}
+
 }  // namespace sg

@@ -27,6 +27,15 @@ __global__ void build_logtab_kernel(double *lntab, int idx0, int n) {
     lntab[i] = -log(c);
 }
 
+__global__ void build_lnint_kernel(double *lnint, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) lnint[i] = i ? log(double(i)) : 0.0;
+}
+
+void launch_build_lnint(const DevLayout &d, cudaStream_t s) {
+    if (d.lnint_n > 0) build_lnint_kernel<<<(d.lnint_n + 255) / 256, 256, 0, s>>>(d.lnint, d.lnint_n);
+}
+
 void launch_build_logtab(const DevLayout &d, cudaStream_t s) {
     build_logtab_kernel<<<(d.tab_entries + 255) / 256, 256, 0, s>>>(d.lntab, d.tab_idx0, d.tab_entries);
 }
@@ -282,7 +291,7 @@ __global__ void finalise_kernel(const double2 *__restrict__ tgt, const int32_t *
                                 const double *__restrict__ TBy, int nX, int nY,
                                 const double *__restrict__ part, int n_split, int64_t first, int64_t count,
                                 double G, double *__restrict__ Fx, double *__restrict__ Fy,
-                                unsigned int *__restrict__ queue) {
+                                unsigned int *__restrict__ queue, const double *__restrict__ lnint, int lnint_n) {
     const int64_t lt = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (lt == 0) { queue[0] = 0u; queue[1] = 0u; }   // drained by this call's interaction kernels; ready for the next
     if (lt >= count) return;
@@ -298,13 +307,13 @@ __global__ void finalise_kernel(const double2 *__restrict__ tgt, const int32_t *
     double sx = 0.0;
     for (int c = 0; c < nX; ++c) {
         const int d = colX[c] - kx;
-        if (d != 0) sx = fma(log(double(abs(d))), bx[c], sx);
+        sx = fma(ln_lattice(d, lnint, lnint_n), bx[c], sx);
     }
     const double *by = TBy + int64_t(itx[t]) * nY;
     double sy = 0.0;
     for (int r = 0; r < nY; ++r) {
         const int d = rowY[r] - ky;
-        if (d != 0) sy = fma(log(double(abs(d))), by[r], sy);
+        sy = fma(ln_lattice(d, lnint, lnint_n), by[r], sy);
     }
     Fx[lt] = -G * (mx + 2.0 * sx);
     Fy[lt] = -G * (my + 2.0 * sy);
@@ -314,7 +323,7 @@ void launch_finalise(const DevLayout &d, const ForcePlan &p, double *Fx, double 
     if (p.count == 0) return;
     finalise_kernel<<<unsigned((p.count + 127) / 128), 128, 0, s>>>(d.tgt, d.itx, d.ity, d.colX, d.rowY, d.TBx, d.TBy,
                                                                    d.nX, d.nY, d.part, p.n_split, p.first, p.count,
-                                                                   d.G, Fx, Fy, d.queue);
+                                                                   d.G, Fx, Fy, d.queue, d.lnint, d.lnint_n);
 }
 
 // ------------------------------------------------------------------------------------------------

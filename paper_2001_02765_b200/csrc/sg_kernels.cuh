@@ -44,7 +44,11 @@ struct DevLayout {
     // split-source partial sums [n_split][2][count]
     double *part = nullptr;
     int64_t part_capacity = 0;        // doubles
-    unsigned int *queue = nullptr;    // work-item counter of the interaction kernel (reset by finalise)
+    unsigned int *queue = nullptr;    // work-item counters of the interaction kernels (reset by finalise)
+    // ln of the integer lattice distances 0 .. lnint_n-1 (lnint[0] = 0) for the separable part; lnint_n = 0 when
+    // the lattice is too large for a table (then finalise calls log())
+    double *lnint = nullptr;
+    int lnint_n = 0;
 };
 
 struct ForcePlan {
@@ -61,6 +65,7 @@ size_t interaction_smem_bytes(int tab_entries);
 cudaError_t configure_kernels(int tab_entries);   // cudaFuncSetAttribute for the opt-in smem size
 
 void launch_build_logtab(const DevLayout &d, cudaStream_t s);
+void launch_build_lnint(const DevLayout &d, cudaStream_t s);
 void launch_fill_static_tiles(const DevLayout &d, cudaStream_t s);        // xc and y of vtile (once)
 void launch_vertex_weights(const DevLayout &d, const double *sigma, cudaStream_t s);
 void launch_line_tables(const DevLayout &d, cudaStream_t s);

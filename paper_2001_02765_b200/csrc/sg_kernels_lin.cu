@@ -246,7 +246,8 @@ __global__ void finalise_lin_kernel(const double2 *__restrict__ tgt, const int32
                                     const double *__restrict__ TBy3, int nX, int nY,
                                     const double *__restrict__ part, int n_split, int64_t first, int64_t count,
                                     double G, double *__restrict__ Fx, double *__restrict__ Fy,
-                                    unsigned int *__restrict__ queue) {
+                                    unsigned int *__restrict__ queue, const double *__restrict__ lnint,
+                                    int lnint_n) {
     const int64_t lt = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (lt == 0) *queue = 0u;
     if (lt >= count) return;
@@ -263,7 +264,7 @@ __global__ void finalise_lin_kernel(const double2 *__restrict__ tgt, const int32
     for (int c = 0; c < nX; ++c) {
         const int d = colX[c] - kx;
         if (d != 0) {
-            const double ln = log(double(abs(d))), dd = double(d);
+            const double ln = ln_lattice(d, lnint, lnint_n), dd = double(d);
             sx = fma(-2.0 * ln, bx[3 * c] + p.y * bx[3 * c + 1] - dd * bx[3 * c + 2], sx);
             sy = fma(2.0 * dd * ln, bx[3 * c + 1], sy);
         }
@@ -272,7 +273,7 @@ __global__ void finalise_lin_kernel(const double2 *__restrict__ tgt, const int32
     for (int r = 0; r < nY; ++r) {
         const int d = rowY[r] - ky;
         if (d != 0) {
-            const double ln = log(double(abs(d))), dd = double(d);
+            const double ln = ln_lattice(d, lnint, lnint_n), dd = double(d);
             sy = fma(-2.0 * ln, by[3 * r] + p.x * by[3 * r + 1] - dd * by[3 * r + 2], sy);
             sx = fma(2.0 * dd * ln, by[3 * r + 1], sx);
         }
@@ -286,7 +287,7 @@ void launch_finalise_lin(const DevLayout &d, const LinArrays &l, const ForcePlan
     if (p.count == 0) return;
     finalise_lin_kernel<<<unsigned((p.count + 127) / 128), 128, 0, s>>>(d.tgt, d.itx, d.ity, d.colX, d.rowY, l.TBx3,
                                                                        l.TBy3, d.nX, d.nY, d.part, p.n_split, p.first,
-                                                                       p.count, d.G, Fx, Fy, d.queue);
+                                                                       p.count, d.G, Fx, Fy, d.queue, d.lnint, d.lnint_n);
 }
 
 }  // namespace sg
