@@ -321,7 +321,7 @@ def run_ours(args):
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>", None)
         elif lattice:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps,
-                                   "patch_same_level_kernel (+ patch_interaction_kernel on multi-level layouts)", None)
+                                   "patch_offset_kernel (+ patch_interaction_kernel on multi-level layouts)", None)
         else:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, direct_name, direct_traffic)
         line = {

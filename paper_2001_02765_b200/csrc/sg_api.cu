@@ -1,5 +1,6 @@
 // sg_api.cu -- the C ABI of include/sg_disk.h: context ownership, uploads, launch planning.
 #include <algorithm>
+#include <climits>
 #include <cmath>
 #include <cstring>
 #include <string>
@@ -21,6 +22,7 @@ struct sg_ctx {
     bool linear = false;         // last density call carried slopes (sg_set_density_linear)
     LinArrays lin;
     PatchArrays patch;           // lattice-offset reuse path (P = 8 or 16)
+    std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning)
     bool use_patch = false;      // sg_set_interaction_mode
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
@@ -127,19 +129,21 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
     return pp;
 }
 
-// Blocked same-level kernel: one work item = (group of 8 target patches, split of the source patch list).
-PatchPlan make_blocked_plan(const sg_ctx *c) {
-    PatchPlan pb = make_patch_plan(c);
-    pb.smem = patch_blocked_smem_bytes(c->dev.tab_entries);
-    if (c->count == 0) return pb;
-    const int n_groups = (pb.n_tpatches + 7) / 8, slots = c->sm_count;
-    const int n_patches = c->patch.n_patches;
-    int want = (8 * slots + n_groups - 1) / n_groups;
-    want = std::max(1, std::min(want, std::max(1, n_patches / 8)));
-    pb.patches_per_split = (n_patches + want - 1) / want;
-    pb.n_split = (n_patches + pb.patches_per_split - 1) / pb.patches_per_split;
-    pb.grid = int(std::min<int64_t>(int64_t(pb.n_split) * n_groups, slots));
-    return pb;
+// Blocked same-level kernel: one work item = (group of <= 8 target patches, split of the group's offset box).
+OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
+    OffsetPlan po;
+    if (c->count == 0) return po;
+    const std::vector<PatchGroup> &g = c->patch_groups;
+    const int last_patch = pp.first_patch + pp.n_tpatches - 1;
+    int g0 = 0, g1 = int(g.size()) - 1;
+    while (g0 < int(g.size()) && g[g0].first + g[g0].n <= pp.first_patch) ++g0;
+    while (g1 >= 0 && g[g1].first > last_patch) --g1;
+    po.g_first = g0;
+    po.n_groups = std::max(0, g1 - g0 + 1);
+    const int slots = c->sm_count * 2;
+    po.n_split = std::max(1, std::min(64, (6 * slots + po.n_groups - 1) / std::max(1, po.n_groups)));
+    po.grid = int(std::min<int64_t>(int64_t(po.n_split) * po.n_groups, slots));
+    return po;
 }
 
 int upload_patches(sg_ctx *c) {
@@ -158,9 +162,54 @@ int upload_patches(sg_ctx *c) {
     if ((rc = upload(c, &pa.info, info))) return rc;
     if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
     SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
-    if (pa.P == 16 && patch_blocked_smem_bytes(c->dev.tab_entries) <= size_t(227) * 1024) {
-        SG_CUDA(c, configure_patch_blocked(c->dev.tab_entries));
-        pa.blocked = true;
+    if (pa.P == 16) {
+        // per level: dense map patch position -> patch index; groups of <= 8 consecutive patches with the box of
+        // patch offsets that can reach a source patch of the same level (patch_offset_kernel)
+        std::vector<PatchLevel> lev(size_t(h.n_levels), PatchLevel{0, 0, 0, 0, 0, 0, 0, 0});
+        std::vector<int32_t> pmap;
+        std::vector<PatchGroup> &groups = c->patch_groups;
+        groups.clear();
+        int64_t map_total = 0;
+        size_t p = 0;
+        bool ok = true;
+        while (p < info.size() && ok) {
+            const int L = h.patches[p].level;
+            size_t q = p;
+            int imin = INT32_MAX, imax = INT32_MIN, jmin = INT32_MAX, jmax = INT32_MIN;
+            for (; q < info.size() && h.patches[q].level == L; ++q) {
+                imin = std::min(imin, h.patches[q].i0 / h.P); imax = std::max(imax, h.patches[q].i0 / h.P);
+                jmin = std::min(jmin, h.patches[q].j0 / h.P); jmax = std::max(jmax, h.patches[q].j0 / h.P);
+            }
+            PatchLevel &l = lev[size_t(L)];
+            if (l.n != 0) { ok = false; break; }                          // patches not sorted by level: no map
+            l = PatchLevel{int32_t(p), int32_t(q - p), imin, jmin, imax - imin + 1, jmax - jmin + 1,
+                           int32_t(map_total), info[p].cw};
+            map_total += int64_t(l.npx) * l.npy;
+            if (map_total > (int64_t(1) << 26)) { ok = false; break; }
+            pmap.resize(size_t(map_total), -1);
+            for (size_t r = p; r < q; ++r)
+                pmap[size_t(l.map_off) + size_t(h.patches[r].j0 / h.P - jmin) * l.npx + (h.patches[r].i0 / h.P - imin)] = int32_t(r);
+            for (size_t r = p; r < q; r += 8) {
+                const int n = int(std::min<size_t>(8, q - r));
+                int gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
+                for (int w = 0; w < n; ++w) {
+                    gimin = std::min(gimin, h.patches[r + w].i0 / h.P); gimax = std::max(gimax, h.patches[r + w].i0 / h.P);
+                    gjmin = std::min(gjmin, h.patches[r + w].j0 / h.P); gjmax = std::max(gjmax, h.patches[r + w].j0 / h.P);
+                }
+                const int64_t ndpi = int64_t(imax - gimin) - (imin - gimax) + 1, ndpj = int64_t(jmax - gjmin) - (jmin - gjmax) + 1;
+                if (ndpi * ndpj > (int64_t(1) << 30)) { ok = false; break; }
+                groups.push_back(PatchGroup{L, int32_t(r), n, imin - gimax, int32_t(ndpi), jmin - gjmax, int32_t(ndpj)});
+            }
+            p = q;
+        }
+        if (ok) {
+            if ((rc = upload(c, &pa.levels, lev)) || (rc = upload(c, &pa.groups, groups)) || (rc = upload(c, &pa.pmap, pmap)))
+                return rc;
+            if ((rc = dev_alloc(c, &pa.wQ, int64_t(pa.n_patches) * kPatchQStride))) return rc;
+            pa.n_groups = int(groups.size());
+            SG_CUDA(c, configure_patch_offset());
+            pa.blocked = true;
+        }
     }
     pa.enabled = true;
     return SG_OK;
@@ -346,15 +395,16 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     SG_CUDA(c, cudaSetDevice(c->device));
     ForcePlan p = make_plan(c);
     const bool by_patch = c->use_patch && !c->linear;
-    PatchPlan pp, pb;                      // cross-level / generic kernel, blocked same-level kernel
+    PatchPlan pp;                          // cross-level / generic kernel
+    OffsetPlan po;                         // blocked same-level kernel
     bool blocked = false, cross = true;
     if (by_patch) {
         pp = make_patch_plan(c);
         blocked = c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count;   // small problems: more, lighter CTAs
         if (blocked) {
-            pb = make_blocked_plan(c);
+            po = make_offset_plan(c, pp);
             cross = c->host.n_levels > 1;
-            p.n_split = pb.n_split + (cross ? pp.n_split : 0);
+            p.n_split = po.n_split + (cross ? pp.n_split : 0);
         } else {
             p.n_split = pp.n_split;        // finalise adds p.n_split partial sums per target
         }
@@ -365,9 +415,9 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
     else if (by_patch) {
-        if (blocked) launch_patch_same_level(c->dev, c->patch, pb, c->first, c->count, s);
+        if (blocked) launch_patch_offset(c->dev, c->patch, po, c->first, c->count, s);
         if (cross) launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count,
-                                            c->dev.part + (blocked ? int64_t(pb.n_split) * 2 * c->count : 0),
+                                            c->dev.part + (blocked ? int64_t(po.n_split) * 2 * c->count : 0),
                                             blocked ? 1 : 0, s);
     }
     else launch_interaction(c->dev, p, s);

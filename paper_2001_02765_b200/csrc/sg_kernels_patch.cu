@@ -21,8 +21,10 @@ constexpr int kPatchMaxM = 48;        // table path for |level difference| <= 1:
 
 // per-patch signed vertex weights: vertex (i,j) of patch p is the NE corner of its cell (i-1,j-1) (+), the NW
 // corner of (i,j-1) (-), the SE corner of (i-1,j) (-) and the SW corner of (i,j) (+)   [[.]] of PAPER.md:92
-__global__ void patch_weights_kernel(const double *__restrict__ sigma, double *__restrict__ wP, int P, int wstride,
-                                     int n_patches) {
+// wQ (P = 16 only, may be null): the same weights with rows 18 apart (column 17 zero) so that patch_offset_kernel
+// stages them with aligned 16-byte copies.
+__global__ void patch_weights_kernel(const double *__restrict__ sigma, double *__restrict__ wP, double *__restrict__ wQ,
+                                     int P, int wstride, int n_patches) {
     const int p = blockIdx.x;
     const double *s = sigma + int64_t(p) * P * P;
     for (int e = threadIdx.x; e < wstride; e += blockDim.x) {
@@ -33,13 +35,17 @@ __global__ void patch_weights_kernel(const double *__restrict__ sigma, double *_
             if (i < P && j >= 1) w -= s[(j - 1) * P + i];
             if (i >= 1 && j < P) w -= s[j * P + (i - 1)];
             if (i < P && j < P) w += s[j * P + i];
+            if (wQ) {
+                wQ[int64_t(p) * kPatchQStride + j * (P + 2) + i] = w;
+                if (i == P) wQ[int64_t(p) * kPatchQStride + j * (P + 2) + P + 1] = 0.0;
+            }
         }
         wP[int64_t(p) * wstride + e] = w;
     }
 }
 
 void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s) {
-    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, pa.wP, pa.P, pa.wstride, pa.n_patches);
+    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, pa.wP, pa.wQ, pa.P, pa.wstride, pa.n_patches);
 }
 
 __device__ __forceinline__ double2 pair_terms(double u, double v, const char *tabb, uint32_t keep) {
@@ -86,7 +92,7 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 
         for (int b = b0; b < b1; ++b) {
             const PatchInfo B = info[b];
-            if (skip_same_level && B.level == A.level) continue;   // done by patch_same_level_kernel (CTA-uniform)
+            if (skip_same_level && B.level == A.level) continue;   // done by patch_offset_kernel (CTA-uniform)
             __syncthreads();                                   // previous pair is done with sw / stab2
             for (int e = tid; e < NV; e += NT) sw[e] = wP[int64_t(b) * wstride + e];
             const int dl = A.level - B.level;
@@ -133,38 +139,65 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 }
 
 // ------------------------------------------------------------------------------------------------
-// Same-level patch pairs, P = 16, register-blocked: ONE WARP per target patch, 8 targets per thread
-// (lane = l + 16 kb owns row l, columns 8 kb .. 8 kb + 7), private offset table and weight buffer per warp, no
-// CTA-wide barrier in the pair loop.  With ra = rb = 1 the table column of (vertex i, target k) is i - k + 15, so
-// one loaded T[row][cc] serves the 8 targets of a thread against 8 consecutive vertices: per table load 16 DFMA,
-// the vertex weights slide through an 8-deep register window (w rows are zero-padded by 7 on the left and 8 on the
-// right, which also takes care of the ragged ends).  Table rows are 33 entries apart so that the 8 lanes of an
-// LDS.128 quarter-warp (8 consecutive l = 8 consecutive table rows) hit 8 different 16-byte bank groups.
+// Same-level patch pairs, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
+//
+// The table of a patch pair depends only on the patch offset d = (B - A) in patch units.  A CTA takes a group of up
+// to 8 target patches A_w of one level (one warp each) and walks over the offsets d of the level's bounding box; for
+// each d warp w looks up the source patch B_w = A_w + d in the level's dense patch map (absent: the warp skips this
+// offset).  All 256 threads tabulate T(d) together (4 pair-function evaluations per thread instead of 32 with a
+// table per warp), double-buffered: the table of offset n+1 is built while offset n is consumed, one CTA barrier
+// per offset.  The log table of the pair function is read through L1 (table building is 3 % of the kernel).
+//
+// Correlation: lane = l + 16 kb owns row l, columns 8 kb .. 8 kb + 7 of its target patch (8 targets per thread).
+// With ra = rb = 1 the table column of (vertex i, target k) is i - k + 15, so one loaded T[row][cc] serves the 8
+// targets of a thread against 8 consecutive vertices: 16 DFMA per LDS.128; the vertex weights slide through an
+// 8-deep register window (fully unrolled; the ragged ends are removed at compile time).  Table rows are 33 entries
+// apart so that the 8 lanes of an LDS.128 quarter-warp (8 consecutive table rows) hit 8 different 16-byte bank
+// groups.  Every per-patch sum stays in one accumulator chain (split chains cancel badly).
 // ------------------------------------------------------------------------------------------------
-constexpr int kBlkWarps = 8, kBlkR = 8, kBlkTRow = 33, kBlkT = 32 * kBlkTRow, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
+constexpr int kOffWarps = 8, kBlkR = 8, kBlkTRow = 33, kBlkT = 32 * kBlkTRow, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
 
-__global__ void __launch_bounds__(kBlkWarps * 32, 1)
-patch_same_level_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ wP, int wstride,
-                        const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_patches,
-                        int patches_per_split, int n_split, int first_patch, int n_tpatches, int64_t first,
-                        int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
+__device__ __forceinline__ double fast_ln_g(double a, const double *__restrict__ lntab_g, int tab_idx0, uint32_t keep) {
+    const uint32_t hi = uint32_t(__double2hiint(a));
+    const uint32_t hc = (hi & keep) | kLogHalfBin;
+    const double tv = __ldg(lntab_g + (int(hc >> kLogShift) - tab_idx0));
+    const double c = rcp_approx(__hiloint2double(int(hc), 0));
+    const double f = fma(a, c, -1.0);
+    double s = fma(f, -0.25, 1.0 / 3.0);
+    s = fma(f, s, -0.5);
+    s = fma(f, s, 1.0);
+    return fma(f, s, tv);
+}
+
+__device__ __forceinline__ double2 pair_terms_g(double u, double v, const double *__restrict__ lntab_g, int tab_idx0,
+                                                uint32_t keep) {
+    const double q = fma(u, u, v * v);
+    const double y0 = rsqrt_approx(q);
+    const double t = q * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double r = fma(t, p * e, t);
+    return make_double2(flip_sign_by(fast_ln_g(fabs(v) + r, lntab_g, tab_idx0, keep), v),
+                        flip_sign_by(fast_ln_g(fabs(u) + r, lntab_g, tab_idx0, keep), u));
+}
+
+__global__ void __launch_bounds__(kOffWarps * 32, 2)
+patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
+                    const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
+                    const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int g_first,
+                    int n_groups, int n_split, int64_t first, int64_t count, double *__restrict__ part,
+                    unsigned int *__restrict__ queue, uint32_t keep) {
     constexpr int P = 16;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                                // [warp][32][33]
-    double *sW = reinterpret_cast<double *>(sT + kBlkWarps * kBlkT);                    // [warp][17][32]
-    double *stab = sW + kBlkWarps * kBlkW;                                              // log table
+    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2][32][33] offset tables, double-buffered
+    double *sW = reinterpret_cast<double *>(sT + 2 * kBlkT);               // [warp][17][8 | 17 | 7] weights of B_w
     __shared__ int s_item;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int l = lane & 15, k0 = (lane >> 4) * kBlkR;
 
-    for (int i = tid; i < tab_entries; i += kBlkWarps * 32) stab[i] = lntab_g[i];
-    for (int i = tid; i < kBlkWarps * kBlkW; i += kBlkWarps * 32) sW[i] = 0.0;          // zero padding stays zero
-    __syncthreads();
-    const char *tabb = reinterpret_cast<const char *>(stab) - int64_t(tab_idx0) * 8 - 4;
-    double2 *T = sT + warp * kBlkT;
+    for (int i = tid; i < kOffWarps * kBlkW; i += kOffWarps * 32) sW[i] = 0.0;           // the padding stays zero
     double *W = sW + warp * kBlkW;
 
-    const int n_groups = (n_tpatches + kBlkWarps - 1) / kBlkWarps;
     const int n_items = n_groups * n_split;
     while (true) {
         __syncthreads();
@@ -172,77 +205,121 @@ patch_same_level_kernel(const PatchInfo *__restrict__ info, const double *__rest
         __syncthreads();
         const int item = s_item;
         if (item >= n_items) break;
-        const int grp = item / n_split, sp = item - grp * n_split;
-        const int ta = grp * kBlkWarps + warp;
-        if (ta >= n_tpatches) continue;                        // whole warp: nothing to do in this group
-        const PatchInfo A = info[first_patch + ta];
-        const int b0 = sp * patches_per_split, b1 = min(n_patches, b0 + patches_per_split);
+        const int gi = item / n_split, sp = item - gi * n_split;
+        const PatchGroup grp = groups[g_first + gi];
+        const PatchLevel lev = levels[grp.level];
+        const int n_off = grp.ndpi * grp.ndpj, per = (n_off + n_split - 1) / n_split;
+        const int n0 = sp * per, n1 = min(n_off, n0 + per);
+        const double g = double(lev.cw);
+
+        // lane w < grp.n of every warp holds the patch position of target patch A_w (for the map look-ups)
+        int api = 0, apj = 0;
+        if (lane < grp.n) {
+            const PatchInfo A = info[grp.first + lane];
+            api = A.X0 / (P * lev.cw) - lev.pimin;
+            apj = A.Y0 / (P * lev.cw) - lev.pjmin;
+        }
+        const bool have_a = warp < grp.n;
         double ax[kBlkR], ay[kBlkR];
 #pragma unroll
         for (int r = 0; r < kBlkR; ++r) { ax[r] = 0.0; ay[r] = 0.0; }
 
-        for (int b = b0; b < b1; ++b) {
-            const PatchInfo B = info[b];
-            if (B.level != A.level) continue;                  // other levels: patch_interaction_kernel
-            __syncwarp();
-            for (int e = lane; e < (P + 1) * (P + 1); e += 32) {
-                const int i = e % (P + 1), j = e / (P + 1);
-                W[j * kBlkWRow + 7 + i] = wP[int64_t(b) * wstride + e];
+        // source patch of this warp at offset n (or -1), and whether any warp of the CTA has one
+        auto lookup = [&](int n, bool &any) -> int {
+            int b = -1;
+            if (n < n1 && lane < grp.n) {
+                const int bi = api + grp.dpi_min + n % grp.ndpi, bj = apj + grp.dpj_min + n / grp.ndpi;
+                if (bi >= 0 && bi < lev.npx && bj >= 0 && bj < lev.npy) b = pmap[lev.map_off + bj * lev.npx + bi];
             }
-            const int g = A.cw, u00 = B.X0 - (A.X0 + g / 2), v00 = B.Y0 - (A.Y0 + g / 2);
-#pragma unroll 4
-            for (int e = lane; e < 32 * 32; e += 32) {
-                const int mm = e & 31, nn = e >> 5;
-                T[nn * kBlkTRow + mm] = pair_terms(double(u00 + (mm - 15) * g), double(v00 + (nn - 15) * g), tabb, keep);
+            any = __ballot_sync(0xffffffffu, b >= 0) != 0u;
+            return __shfl_sync(0xffffffffu, b, warp & 7);
+        };
+        auto build = [&](int n, double2 *T) {
+            const double u00 = double((grp.dpi_min + n % grp.ndpi) * P) * g - 0.5 * g;
+            const double v00 = double((grp.dpj_min + n / grp.ndpi) * P) * g - 0.5 * g;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int e = tid + q * (kOffWarps * 32), mm = e & 31, nn = e >> 5;
+                T[nn * kBlkTRow + mm] = pair_terms_g(fma(double(mm - 15), g, u00), fma(double(nn - 15), g, v00),
+                                                     lntab_g, tab_idx0, keep);
             }
-            __syncwarp();
-            const int cbase = 8 - k0;
-            for (int j = 0; j <= P; ++j) {
-                const double2 *trow = T + (j - l + 15) * kBlkTRow + cbase;
-                const double *wrow = W + j * kBlkWRow;
-                double win[8];
+        };
+
+        bool any_cur, any_next = false;
+        int b_cur = lookup(n0, any_cur), b_next = -1;
+        if (any_cur) build(n0, sT);
+        __syncthreads();
+        for (int n = n0; n < n1; ++n) {
+            b_next = lookup(n + 1, any_next);
+            if (!any_cur && !any_next) continue;                 // nothing built, nothing consumed: no barrier needed
+            if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * kBlkT);
+            if (have_a && b_cur >= 0) {
+                // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 + 17 + 7]
+                const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b_cur) * kPatchQStride);
+                __syncwarp();
 #pragma unroll
-                for (int r = 0; r < 7; ++r) win[r] = wrow[r];
+                for (int q = 0; q < 5; ++q) {
+                    const int e2 = lane + 32 * q;
+                    if (e2 < 17 * 9) {
+                        const int j = e2 / 9, c2 = e2 - 9 * j;
+                        *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
+                    }
+                }
+                __syncwarp();
+                const double2 *T = sT + ((n - n0) & 1) * kBlkT;
+                const int cbase = 8 - k0;
+#pragma unroll 1
+                for (int j = 0; j <= P; ++j) {
+                    const double2 *trow = T + (j - l + 15) * kBlkTRow + cbase;
+                    const double *wrow = W + j * kBlkWRow + 1;            // wrow[7 + i] = weight of vertex i
+                    double wv[P + 2];                                     // compile-time indices only: registers
 #pragma unroll
-                for (int t = 0; t < P + kBlkR; ++t) {
-                    win[(t + 7) & 7] = wrow[t + 7];
-                    const double2 Tv = trow[t];
+                    for (int t = 0; t < P + kBlkR; ++t) {
+                        if ((t & 1) == 0 && t <= P) {                     // vertices t, t+1 (column 17 is zero padding)
+                            const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t + 7);
+                            wv[t] = w2.x;
+                            wv[t + 1] = w2.y;
+                        }
+                        const double2 Tv = trow[t];
 #pragma unroll
-                    for (int r = 0; r < kBlkR; ++r) {
-                        if (t + r >= 7 && t + r <= 7 + P) {      // vertex i = t + r - 7 exists (compile-time)
-                            ax[r] = fma(win[(t + r) & 7], Tv.x, ax[r]);
-                            ay[r] = fma(win[(t + r) & 7], Tv.y, ay[r]);
+                        for (int r = 0; r < kBlkR; ++r) {
+                            if (t + r >= 7 && t + r <= 7 + P) {      // vertex i = t + r - 7 exists (compile-time)
+                                ax[r] = fma(wv[t + r - 7], Tv.x, ax[r]);
+                                ay[r] = fma(wv[t + r - 7], Tv.y, ay[r]);
+                            }
                         }
                     }
                 }
             }
+            __syncthreads();
+            b_cur = b_next; any_cur = any_next;
         }
+        if (have_a) {
 #pragma unroll
-        for (int r = 0; r < kBlkR; ++r) {
-            const int64_t lt = (int64_t(first_patch + ta) * (P * P) + l * P + k0 + r) - first;
-            if (lt >= 0 && lt < count) {
-                part[(int64_t(sp) * 2 + 0) * count + lt] = ax[r];
-                part[(int64_t(sp) * 2 + 1) * count + lt] = ay[r];
+            for (int r = 0; r < kBlkR; ++r) {
+                const int64_t lt = (int64_t(grp.first + warp) * (P * P) + l * P + k0 + r) - first;
+                if (lt >= 0 && lt < count) {
+                    part[(int64_t(sp) * 2 + 0) * count + lt] = ax[r];
+                    part[(int64_t(sp) * 2 + 1) * count + lt] = ay[r];
+                }
             }
         }
     }
 }
 
-size_t patch_blocked_smem_bytes(int tab_entries) {
-    return size_t(kBlkWarps) * (kBlkT * 16 + kBlkW * 8) + size_t(tab_entries) * 8;
+size_t patch_offset_smem_bytes() { return size_t(2) * kBlkT * 16 + size_t(kOffWarps) * kBlkW * 8; }
+
+cudaError_t configure_patch_offset() {
+    return cudaFuncSetAttribute(patch_offset_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(patch_offset_smem_bytes()));
 }
 
-cudaError_t configure_patch_blocked(int tab_entries) {
-    return cudaFuncSetAttribute(patch_same_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(patch_blocked_smem_bytes(tab_entries)));
-}
-
-void launch_patch_same_level(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                             int64_t count, cudaStream_t s) {
-    if (count == 0) return;
-    patch_same_level_kernel<<<pp.grid, kBlkWarps * 32, pp.smem, s>>>(
-        pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split, pp.n_split,
-        pp.first_patch, pp.n_tpatches, first, count, d.part, d.queue + 1, kLogKeepMask);
+void launch_patch_offset(const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first, int64_t count,
+                         cudaStream_t s) {
+    if (count == 0 || po.n_groups == 0) return;
+    patch_offset_kernel<<<po.grid, kOffWarps * 32, patch_offset_smem_bytes(), s>>>(pa.info, pa.levels, pa.groups, pa.pmap, pa.wQ, d.lntab,
+                                                          d.tab_idx0, po.g_first, po.n_groups, po.n_split, first,
+                                                          count, d.part, d.queue + 1, kLogKeepMask);
 }
 
 size_t patch_smem_bytes(int P, int tab_entries) {

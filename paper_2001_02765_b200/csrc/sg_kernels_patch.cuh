@@ -10,9 +10,28 @@ struct PatchInfo {                    // one leaf patch on the integer lattice
     int32_t level;
 };
 
+struct PatchLevel {                   // the leaf patches of one level (contiguous in the sorted patch list)
+    int32_t p0, n;                    // patches [p0, p0 + n)
+    int32_t pimin, pjmin, npx, npy;   // bounding box of their positions in patch units (i0 / P, j0 / P)
+    int32_t map_off;                  // pmap[map_off + (pj - pjmin) * npx + (pi - pimin)] = patch index or -1
+    int32_t cw;                       // cell width in lattice units
+};
+
+struct PatchGroup {                   // <= 8 consecutive target patches of one level: one CTA work item per split
+    int32_t level, first, n;
+    int32_t dpi_min, ndpi, dpj_min, ndpj;   // box of patch offsets d = B - A that can hit a source patch of the level
+};
+
+constexpr int kPatchQStride = 17 * 18;   // doubles per patch in wQ
+
 struct PatchArrays {
     bool enabled = false;             // P is 8 or 16
-    bool blocked = false;             // P == 16 and the per-warp tables + log table fit in shared memory
+    bool blocked = false;             // P == 16: patch_offset_kernel available (dense per-level patch maps built)
+    PatchLevel *levels = nullptr;     // [n_levels]
+    PatchGroup *groups = nullptr;     // [n_groups], ordered by first patch
+    int n_groups = 0;
+    int32_t *pmap = nullptr;
+    double *wQ = nullptr;             // [n_patches * kPatchQStride] per-patch weights, rows 18 apart
     int P = 0;
     int n_patches = 0;
     int wstride = 0;                  // doubles per patch in wP: (P+1)^2 rounded up to a multiple of 2
@@ -32,10 +51,16 @@ cudaError_t configure_patch_kernels(int P, int tab_entries);
 void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s);
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
                               int64_t count, double *part, int skip_same_level, cudaStream_t s);
-// register-blocked same-level kernel (P = 16); uses the second queue counter (d.queue + 1), writes d.part slots
-size_t patch_blocked_smem_bytes(int tab_entries);
-cudaError_t configure_patch_blocked(int tab_entries);
-void launch_patch_same_level(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                             int64_t count, cudaStream_t s);
+// register-blocked same-level kernel with one offset table per CTA (P = 16); uses the second queue counter
+// (d.queue + 1) and writes the first po.n_split slots of d.part
+struct OffsetPlan {
+    int g_first = 0, n_groups = 0;    // groups touched by the target range
+    int n_split = 1;                  // splits of every group's offset list
+    int grid = 0;
+};
+size_t patch_offset_smem_bytes();
+cudaError_t configure_patch_offset();
+void launch_patch_offset(const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first, int64_t count,
+                         cudaStream_t s);
 
 }  // namespace sg
