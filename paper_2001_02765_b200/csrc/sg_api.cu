@@ -22,7 +22,8 @@ struct sg_ctx {
     bool linear = false;         // last density call carried slopes (sg_set_density_linear)
     LinArrays lin;
     PatchArrays patch;           // lattice-offset reuse path (P = 8 or 16)
-    std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning)
+    std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning): list 0 then list 1
+    int patch_n_groups0 = 0;                // groups of list 0 (pair classes "same level", "finer source")
     bool use_patch = false;      // sg_set_interaction_mode
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
@@ -129,20 +130,24 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
     return pp;
 }
 
-// Blocked same-level kernel: one work item = (group of <= 8 target patches, split of the group's offset box).
+// Blocked kernels (patch pairs at most one level apart): one work item = (group of <= 8 target patches, split of the
+// group's offset box), per pair class.
 OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
     OffsetPlan po;
     if (c->count == 0) return po;
-    const std::vector<PatchGroup> &g = c->patch_groups;
-    const int last_patch = pp.first_patch + pp.n_tpatches - 1;
-    int g0 = 0, g1 = int(g.size()) - 1;
-    while (g0 < int(g.size()) && g[g0].first + g[g0].n <= pp.first_patch) ++g0;
-    while (g1 >= 0 && g[g1].first > last_patch) --g1;
-    po.g_first = g0;
-    po.n_groups = std::max(0, g1 - g0 + 1);
+    po.n_groups0 = c->patch_n_groups0;
+    po.n_groups1 = int(c->patch_groups.size()) - po.n_groups0;
+    po.first_patch = pp.first_patch;
+    po.last_patch = pp.first_patch + pp.n_tpatches - 1;
+    int touched = 0;
+    for (size_t i = 0; i < c->patch_groups.size(); ++i) {
+        const PatchGroup &g = c->patch_groups[i];
+        if (g.pmax < po.first_patch || g.pmin > po.last_patch) continue;
+        if (int(i) < po.n_groups0) ++touched;
+        for (int v = 0; v < 3; ++v) po.variant[v] = po.variant[v] || g.box[v][1] > 0;
+    }
     const int slots = c->sm_count * 2;
-    po.n_split = std::max(1, std::min(64, (6 * slots + po.n_groups - 1) / std::max(1, po.n_groups)));
-    po.grid = int(std::min<int64_t>(int64_t(po.n_split) * po.n_groups, slots));
+    po.n_split = std::max(1, std::min(64, (6 * slots + touched - 1) / std::max(1, touched)));
     return po;
 }
 
@@ -189,19 +194,66 @@ int upload_patches(sg_ctx *c) {
             pmap.resize(size_t(map_total), -1);
             for (size_t r = p; r < q; ++r)
                 pmap[size_t(l.map_off) + size_t(h.patches[r].j0 / h.P - jmin) * l.npx + (h.patches[r].i0 / h.P - imin)] = int32_t(r);
-            for (size_t r = p; r < q; r += 8) {
-                const int n = int(std::min<size_t>(8, q - r));
-                int gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
-                for (int w = 0; w < n; ++w) {
-                    gimin = std::min(gimin, h.patches[r + w].i0 / h.P); gimax = std::max(gimax, h.patches[r + w].i0 / h.P);
-                    gjmin = std::min(gjmin, h.patches[r + w].j0 / h.P); gjmax = std::max(gjmax, h.patches[r + w].j0 / h.P);
-                }
-                const int64_t ndpi = int64_t(imax - gimin) - (imin - gimax) + 1, ndpj = int64_t(jmax - gjmin) - (jmin - gjmax) + 1;
-                if (ndpi * ndpj > (int64_t(1) << 30)) { ok = false; break; }
-                groups.push_back(PatchGroup{L, int32_t(r), n, imin - gimax, int32_t(ndpi), jmin - gjmax, int32_t(ndpj)});
-            }
             p = q;
         }
+        // groups of 8 target patches in sorted order with their offset boxes.  List 0 (any patches of a level) serves
+        // the pair classes "same level" and "finer source"; list 1 (patches of one parity class (pi % 2, pj % 2))
+        // serves "coarser source", where A + d must be even for the whole group.
+        std::vector<PatchGroup> glist[2];
+        for (int L = 0; L < h.n_levels && ok; ++L) {
+            const PatchLevel &l = lev[size_t(L)];
+            if (l.n == 0) continue;
+            for (int cls = -1; cls < 4; ++cls) {                       // -1: list 0
+                if (cls >= 0 && (L == 0 || lev[size_t(L - 1)].n == 0)) break;
+                std::vector<int32_t> members;
+                for (int32_t r = l.p0; r < l.p0 + l.n; ++r)
+                    if (cls < 0 || (((h.patches[size_t(r)].i0 / h.P) & 1) == (cls & 1) && ((h.patches[size_t(r)].j0 / h.P) & 1) == (cls >> 1)))
+                        members.push_back(r);
+                for (size_t m0 = 0; m0 < members.size() && ok; m0 += 8) {
+                    PatchGroup gr;
+                    std::memset(&gr, 0, sizeof gr);
+                    gr.level = L;
+                    gr.n = int(std::min<size_t>(8, members.size() - m0));
+                    int gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
+                    gr.pmin = INT32_MAX; gr.pmax = INT32_MIN;
+                    for (int w = 0; w < 8; ++w) {
+                        gr.patch[w] = w < gr.n ? members[m0 + size_t(w)] : -1;
+                        if (w >= gr.n) continue;
+                        const sg_patch &q = h.patches[size_t(gr.patch[w])];
+                        gimin = std::min(gimin, q.i0 / h.P); gimax = std::max(gimax, q.i0 / h.P);
+                        gjmin = std::min(gjmin, q.j0 / h.P); gjmax = std::max(gjmax, q.j0 / h.P);
+                        gr.pmin = std::min(gr.pmin, gr.patch[w]); gr.pmax = std::max(gr.pmax, gr.patch[w]);
+                    }
+                    // d ranges over [lo, hi] per axis; the coarser-source class keeps the parity of the patch positions
+                    auto set_box = [&](int v, int64_t lox, int64_t hix, int64_t loy, int64_t hiy, int step) {
+                        if (step == 2) {
+                            if ((lox & 1) != (cls & 1)) ++lox;
+                            if ((loy & 1) != (cls >> 1)) ++loy;
+                        }
+                        const int64_t nx = hix >= lox ? (hix - lox) / step + 1 : 0, ny = hiy >= loy ? (hiy - loy) / step + 1 : 0;
+                        if (nx * ny > (int64_t(1) << 30)) { ok = false; return; }
+                        gr.box[v][0] = int32_t(lox); gr.box[v][1] = int32_t(nx * ny > 0 ? nx : 0);
+                        gr.box[v][2] = int32_t(loy); gr.box[v][3] = int32_t(nx * ny > 0 ? ny : 0);
+                    };
+                    if (cls < 0) {
+                        set_box(kOffSame, l.pimin - gimax, l.pimin + l.npx - 1 - gimin, l.pjmin - gjmax, l.pjmin + l.npy - 1 - gjmin, 1);
+                        if (L + 1 < h.n_levels && lev[size_t(L + 1)].n > 0) {   // 2 A + d inside the finer level's box
+                            const PatchLevel &f0 = lev[size_t(L + 1)];
+                            set_box(kOffFinerSrc, int64_t(f0.pimin) - 2 * int64_t(gimax), int64_t(f0.pimin + f0.npx - 1) - 2 * int64_t(gimin),
+                                    int64_t(f0.pjmin) - 2 * int64_t(gjmax), int64_t(f0.pjmin + f0.npy - 1) - 2 * int64_t(gjmin), 1);
+                        }
+                    } else {                                           // (A + d) / 2 inside the coarser level's box
+                        const PatchLevel &c0 = lev[size_t(L - 1)];
+                        set_box(kOffCoarserSrc, 2 * int64_t(c0.pimin) - gimax, 2 * int64_t(c0.pimin + c0.npx - 1) - gimin,
+                                2 * int64_t(c0.pjmin) - gjmax, 2 * int64_t(c0.pjmin + c0.npy - 1) - gjmin, 2);
+                    }
+                    glist[cls < 0 ? 0 : 1].push_back(gr);
+                }
+            }
+        }
+        groups = glist[0];
+        c->patch_n_groups0 = int(glist[0].size());
+        groups.insert(groups.end(), glist[1].begin(), glist[1].end());
         if (ok) {
             if ((rc = upload(c, &pa.levels, lev)) || (rc = upload(c, &pa.groups, groups)) || (rc = upload(c, &pa.pmap, pmap)))
                 return rc;
@@ -239,8 +291,8 @@ int upload_layout(sg_ctx *c) {
     if ((rc = upload(c, &d.rowY, h.rowY)) || (rc = upload(c, &d.rowstart, h.rowstart))) return rc;
     if ((rc = upload(c, &d.rowperm, h.rowperm))) return rc;
     if ((rc = upload(c, &d.chunk_x, h.chunk_x)) || (rc = upload(c, &d.slot_vertex, h.slot_vertex))) return rc;
-    if ((rc = dev_alloc(c, &d.queue, 2))) return rc;
-    SG_CUDA(c, cudaMemset(d.queue, 0, 2 * sizeof(unsigned int)));
+    if ((rc = dev_alloc(c, &d.queue, kQueues))) return rc;
+    SG_CUDA(c, cudaMemset(d.queue, 0, kQueues * sizeof(unsigned int)));
     if ((rc = upload(c, &d.tX, h.tX)) || (rc = upload(c, &d.tY, h.tY))) return rc;
     if ((rc = dev_alloc(c, &d.vtile, int64_t(d.n_tiles) * kTileDoubles))) return rc;
     if ((rc = dev_alloc(c, &d.w, h.Nv))) return rc;
@@ -395,18 +447,19 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     SG_CUDA(c, cudaSetDevice(c->device));
     ForcePlan p = make_plan(c);
     const bool by_patch = c->use_patch && !c->linear;
-    PatchPlan pp;                          // cross-level / generic kernel
-    OffsetPlan po;                         // blocked same-level kernel
-    bool blocked = false, cross = true;
+    PatchPlan pp;                          // generic kernel: everything (small problems) or pairs >= 2 levels apart
+    OffsetPlan po;                         // blocked kernels: pairs at most one level apart
+    bool blocked = false, far = true;
     if (by_patch) {
         pp = make_patch_plan(c);
         blocked = c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count;   // small problems: more, lighter CTAs
         if (blocked) {
             po = make_offset_plan(c, pp);
-            cross = c->host.n_levels > 1;
-            p.n_split = po.n_split + (cross ? pp.n_split : 0);
+            far = c->host.n_levels > 2;
+            const int nv = int(po.variant[0]) + int(po.variant[1]) + int(po.variant[2]);
+            p.n_split = nv * po.n_split + (far ? pp.n_split : 0);  // finalise adds p.n_split partial sums per target
         } else {
-            p.n_split = pp.n_split;        // finalise adds p.n_split partial sums per target
+            p.n_split = pp.n_split;
         }
     }
     int rc = ensure_partials(c, p);
@@ -415,10 +468,15 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
     else if (by_patch) {
-        if (blocked) launch_patch_offset(c->dev, c->patch, po, c->first, c->count, s);
-        if (cross) launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count,
-                                            c->dev.part + (blocked ? int64_t(po.n_split) * 2 * c->count : 0),
-                                            blocked ? 1 : 0, s);
+        double *part = c->dev.part;        // every launch writes its own n_split slots of [2][count] partial sums
+        if (blocked)
+            for (int v = 0; v < 3; ++v)
+                if (po.variant[v]) {
+                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, s);
+                    part += int64_t(po.n_split) * 2 * c->count;
+                }
+        if (!blocked || far)
+            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 2 : 0, s);
     }
     else launch_interaction(c->dev, p, s);
     if (c->timing) {
@@ -458,7 +516,10 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
         int n = 1;
         if (c->use_patch && !c->linear && c->count > 0) {
             const PatchPlan pp = make_patch_plan(c);
-            if (c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count && c->host.n_levels > 1) n = 2;
+            if (c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count) {
+                const OffsetPlan po = make_offset_plan(c, pp);
+                n = int(po.variant[0]) + int(po.variant[1]) + int(po.variant[2]) + (c->host.n_levels > 2 ? 1 : 0);
+            }
         }
         *force_launches = c->count > 0 ? n + 1 : 0;
     }

@@ -293,7 +293,7 @@ __global__ void finalise_kernel(const double2 *__restrict__ tgt, const int32_t *
                                 double G, double *__restrict__ Fx, double *__restrict__ Fy,
                                 unsigned int *__restrict__ queue, const double *__restrict__ lnint, int lnint_n) {
     const int64_t lt = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (lt == 0) { queue[0] = 0u; queue[1] = 0u; }   // drained by this call's interaction kernels; ready for the next
+    if (lt < kQueues) queue[lt] = 0u;                 // drained by this call's interaction kernels; ready for the next
     if (lt >= count) return;
     const int64_t t = first + lt;
     const double2 p = tgt[t];

@@ -15,6 +15,7 @@ constexpr int kTileSlots = kChunksPerTile * kChunk;              // 256 vertex s
 constexpr int kTileDoubles = kChunksPerTile + 2 * kTileSlots;    // 528 doubles
 constexpr int kStages = 3;            // tiles in flight per CTA
 constexpr int kThreads = 256;         // threads per CTA of the interaction kernel
+constexpr int kQueues = 8;            // atomic work-item counters per context
 constexpr int kLogK = 9;              // mantissa bits in the log-table index (|f| <= 2^-10 -> degree 4)
 
 struct DevLayout {
@@ -44,7 +45,7 @@ struct DevLayout {
     // split-source partial sums [n_split][2][count]
     double *part = nullptr;
     int64_t part_capacity = 0;        // doubles
-    unsigned int *queue = nullptr;    // work-item counters of the interaction kernels (reset by finalise)
+    unsigned int *queue = nullptr;    // kQueues work-item counters of the interaction kernels (reset by finalise)
     // ln of the integer lattice distances 0 .. lnint_n-1 (lnint[0] = 0) for the separable part; lnint_n = 0 when
     // the lattice is too large for a table (then finalise calls log())
     double *lnint = nullptr;

@@ -12,6 +12,8 @@
 //     M^x[l][k] += sum_{j,i} w^B[j][i] T[j rb - l ra][i rb - k ra].x          (2 DFMA per pair)
 // Patch pairs more than one level apart (large M) are summed directly, pair by pair, in the same kernel.
 // The separable ln|u| part, the coincidence rule and the epilogue are unchanged (finalise_kernel).
+#include <algorithm>
+
 #include "sg_device.cuh"
 #include "sg_kernels_patch.cuh"
 
@@ -65,7 +67,7 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
                          const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_patches,
                          int patches_per_split, int n_split, int first_patch, int n_tpatches, int64_t first,
                          int64_t count, double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep,
-                         int skip_same_level) {
+                         int skip_near) {
     constexpr int NT = P * P, NV = (P + 1) * (P + 1);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2 *stab2 = reinterpret_cast<double2 *>(smem_raw);                        // kPatchMaxM^2 pair table
@@ -92,7 +94,7 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 
         for (int b = b0; b < b1; ++b) {
             const PatchInfo B = info[b];
-            if (skip_same_level && B.level == A.level) continue;   // done by patch_offset_kernel (CTA-uniform)
+            if (abs(A.level - B.level) < skip_near) continue;     // done by patch_offset_kernel (CTA-uniform)
             __syncthreads();                                   // previous pair is done with sw / stab2
             for (int e = tid; e < NV; e += NT) sw[e] = wP[int64_t(b) * wstride + e];
             const int dl = A.level - B.level;
@@ -139,23 +141,30 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 }
 
 // ------------------------------------------------------------------------------------------------
-// Same-level patch pairs, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
+// Patch pairs at most one level apart, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
 //
-// The table of a patch pair depends only on the patch offset d = (B - A) in patch units.  A CTA takes a group of up
-// to 8 target patches A_w of one level (one warp each) and walks over the offsets d of the level's bounding box; for
-// each d warp w looks up the source patch B_w = A_w + d in the level's dense patch map (absent: the warp skips this
-// offset).  All 256 threads tabulate T(d) together (4 pair-function evaluations per thread instead of 32 with a
-// table per warp), double-buffered: the table of offset n+1 is built while offset n is consumed, one CTA barrier
-// per offset.  The log table of the pair function is read through L1 (table building is 3 % of the kernel).
+// The table of a patch pair depends only on the patch offset d = B - A (in units of the finer level's patch size)
+// and on the pair class V: source level = target level (V = 0), one level coarser (V = 1), one level finer (V = 2).
+// A CTA takes a group of up to 8 target patches A_w of one level (one warp each; all of one parity class
+// (pi % 2, pj % 2), so that for V = 1 the coarse patch at (A_w + d) / 2 exists for all of them or none) and walks over
+// the offsets d of the class's box; for each d warp w looks up its source patch B_w in the source level's dense patch
+// map (absent: the warp skips this offset).  All 256 threads tabulate T(d) together (4-9 pair-function evaluations
+// per thread instead of 32-72 with a table per warp), double-buffered: the table of offset n+1 is built while offset n
+// is consumed, one CTA barrier per offset.  The log table of the pair function is read through L1.
 //
-// Correlation: lane = l + 16 kb owns row l, columns 8 kb .. 8 kb + 7 of its target patch (8 targets per thread).
-// With ra = rb = 1 the table column of (vertex i, target k) is i - k + 15, so one loaded T[row][cc] serves the 8
-// targets of a thread against 8 consecutive vertices: 16 DFMA per LDS.128; the vertex weights slide through an
-// 8-deep register window (fully unrolled; the ragged ends are removed at compile time).  Table rows are 33 entries
-// apart so that the 8 lanes of an LDS.128 quarter-warp (8 consecutive table rows) hit 8 different 16-byte bank
-// groups.  Every per-patch sum stays in one accumulator chain (split chains cancel badly).
+// Correlation, 8 targets per thread, lane = l + 16 h (l = target row).  With vertex (i, j) of B and target (k, l) of A
+// the table entry is T[j rb - l ra + 15 ra][i rb - k ra + 15 ra]:
+//   V = 0 (ra = rb = 1): thread owns columns k = 8 h + r; entry column t + 8 - 8 h serves vertices i = t + r - 7;
+//   V = 1 (ra = 1, rb = 2): thread owns the columns of one parity, k = 2 r + h; entry column 2 t + 1 - h serves i = t + r - 7;
+//   V = 2 (ra = 2, rb = 1): thread owns k = 8 h + r; entry column t + 16 - 16 h serves i = t + 2 r - 14; table rows are
+//          stored even rows first (row j - 2 l + 30 has the parity of j, so the 16 lanes read consecutive stored rows).
+// One loaded entry serves the 8 targets of a thread (16 DFMA per LDS.128); the vertex weights sit in registers
+// (fully unrolled, compile-time indices; the ragged ends are removed at compile time).  Stored table rows are an odd
+// number of entries apart so that the 8 lanes of an LDS.128 quarter-warp hit 8 different 16-byte bank groups.
+// Every per-patch sum stays in one accumulator chain (split chains cancel badly).
 // ------------------------------------------------------------------------------------------------
-constexpr int kOffWarps = 8, kBlkR = 8, kBlkTRow = 33, kBlkT = 32 * kBlkTRow, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
+constexpr int kOffWarps = 8, kBlkR = 8, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
+constexpr int kOffTRowMax = 49, kOffTMax = 48 * kOffTRowMax;            // largest table: V = 1, 48 x 48 entries
 
 __device__ __forceinline__ double fast_ln_g(double a, const double *__restrict__ lntab_g, int tab_idx0, uint32_t keep) {
     const uint32_t hi = uint32_t(__double2hiint(a));
@@ -181,19 +190,26 @@ __device__ __forceinline__ double2 pair_terms_g(double u, double v, const double
                         flip_sign_by(fast_ln_g(fabs(u) + r, lntab_g, tab_idx0, keep), u));
 }
 
+template <int V>
 __global__ void __launch_bounds__(kOffWarps * 32, 2)
 patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
-                    const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int g_first,
-                    int n_groups, int n_split, int64_t first, int64_t count, double *__restrict__ part,
-                    unsigned int *__restrict__ queue, uint32_t keep) {
+                    const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int n_groups,
+                    int n_split, int first_patch, int last_patch, int64_t first, int64_t count,
+                    double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
     constexpr int P = 16;
+    constexpr int RA = V == kOffFinerSrc ? 2 : 1, RB = V == kOffCoarserSrc ? 2 : 1;
+    constexpr int M = P * RB + (P - 1) * RA + 1, MMIN = (P - 1) * RA;     // table side: 32, 48, 47
+    constexpr int TROW = V == kOffSame ? 33 : kOffTRowMax, TBUF = V == kOffSame ? 32 * 33 : kOffTMax;
+    constexpr int STEP = V == kOffCoarserSrc ? 2 : 1;                     // offsets keep A + d even for V = 1
+    constexpr int EVALS = (M * M + kOffWarps * 32 - 1) / (kOffWarps * 32);
+    constexpr int NT = V == kOffFinerSrc ? P + 2 * (kBlkR - 1) + 1 : P + kBlkR;   // table entries per thread and row
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2][32][33] offset tables, double-buffered
-    double *sW = reinterpret_cast<double *>(sT + 2 * kBlkT);               // [warp][17][8 | 17 | 7] weights of B_w
+    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2][TBUF] offset tables, double-buffered
+    double *sW = reinterpret_cast<double *>(sT + 2 * TBUF);                // [warp][17][8 | 18 | 6] weights of B_w
     __shared__ int s_item;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int l = lane & 15, k0 = (lane >> 4) * kBlkR;
+    const int l = lane & 15, h = lane >> 4;
 
     for (int i = tid; i < kOffWarps * kBlkW; i += kOffWarps * 32) sW[i] = 0.0;           // the padding stays zero
     double *W = sW + warp * kBlkW;
@@ -206,20 +222,25 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         const int item = s_item;
         if (item >= n_items) break;
         const int gi = item / n_split, sp = item - gi * n_split;
-        const PatchGroup grp = groups[g_first + gi];
-        const PatchLevel lev = levels[grp.level];
-        const int n_off = grp.ndpi * grp.ndpj, per = (n_off + n_split - 1) / n_split;
+        const PatchGroup *gp = groups + gi;
+        if (gp->pmax < first_patch || gp->pmin > last_patch) continue;          // no target of the range in this group
+        const int grp_n = gp->n, grp_level = gp->level;
+        const PatchLevel lev = levels[grp_level];
+        const int src_level = grp_level + (V == kOffCoarserSrc ? -1 : V == kOffFinerSrc ? 1 : 0);
+        const int dpi_min = gp->box[V][0], ndpi = gp->box[V][1], dpj_min = gp->box[V][2], ndpj = gp->box[V][3];
+        const int n_off = ndpi * ndpj, per = (n_off + n_split - 1) / n_split;   // 0 when the class is absent here
         const int n0 = sp * per, n1 = min(n_off, n0 + per);
-        const double g = double(lev.cw);
+        const PatchLevel slev = levels[n_off > 0 ? src_level : grp_level];
+        const double g = double(min(lev.cw, slev.cw));
 
         // lane w < grp.n of every warp holds the patch position of target patch A_w (for the map look-ups)
         int api = 0, apj = 0;
-        if (lane < grp.n) {
-            const PatchInfo A = info[grp.first + lane];
-            api = A.X0 / (P * lev.cw) - lev.pimin;
-            apj = A.Y0 / (P * lev.cw) - lev.pjmin;
+        if (lane < grp_n) {
+            const PatchInfo A = info[gp->patch[lane]];
+            api = A.X0 / (P * lev.cw);
+            apj = A.Y0 / (P * lev.cw);
         }
-        const bool have_a = warp < grp.n;
+        const int my_patch = warp < grp_n ? gp->patch[warp] : -1;
         double ax[kBlkR], ay[kBlkR];
 #pragma unroll
         for (int r = 0; r < kBlkR; ++r) { ax[r] = 0.0; ay[r] = 0.0; }
@@ -227,34 +248,43 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         // source patch of this warp at offset n (or -1), and whether any warp of the CTA has one
         auto lookup = [&](int n, bool &any) -> int {
             int b = -1;
-            if (n < n1 && lane < grp.n) {
-                const int bi = api + grp.dpi_min + n % grp.ndpi, bj = apj + grp.dpj_min + n / grp.ndpi;
-                if (bi >= 0 && bi < lev.npx && bj >= 0 && bj < lev.npy) b = pmap[lev.map_off + bj * lev.npx + bi];
+            if (n < n1 && lane < grp_n) {
+                const int dx = dpi_min + STEP * (n % ndpi), dy = dpj_min + STEP * (n / ndpi);
+                int bi, bj;
+                if (V == kOffSame) { bi = api + dx; bj = apj + dy; }
+                else if (V == kOffCoarserSrc) { bi = (api + dx) >> 1; bj = (apj + dy) >> 1; }
+                else { bi = 2 * api + dx; bj = 2 * apj + dy; }
+                bi -= slev.pimin; bj -= slev.pjmin;
+                if (bi >= 0 && bi < slev.npx && bj >= 0 && bj < slev.npy) b = pmap[slev.map_off + bj * slev.npx + bi];
             }
             any = __ballot_sync(0xffffffffu, b >= 0) != 0u;
             return __shfl_sync(0xffffffffu, b, warp & 7);
         };
+        // T[row][col] = pair function at u = B.X0 - x_centre(A, k = 0) + (col - MMIN) g, likewise v
         auto build = [&](int n, double2 *T) {
-            const double u00 = double((grp.dpi_min + n % grp.ndpi) * P) * g - 0.5 * g;
-            const double v00 = double((grp.dpj_min + n / grp.ndpi) * P) * g - 0.5 * g;
+            const double u00 = double((dpi_min + STEP * (n % ndpi)) * P) * g - 0.5 * double(lev.cw);
+            const double v00 = double((dpj_min + STEP * (n / ndpi)) * P) * g - 0.5 * double(lev.cw);
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int e = tid + q * (kOffWarps * 32), mm = e & 31, nn = e >> 5;
-                T[nn * kBlkTRow + mm] = pair_terms_g(fma(double(mm - 15), g, u00), fma(double(nn - 15), g, v00),
-                                                     lntab_g, tab_idx0, keep);
+            for (int q = 0; q < EVALS; ++q) {
+                const int e = tid + q * (kOffWarps * 32), mm = e % M, nn = e / M;
+                if (M * M % (kOffWarps * 32) == 0 || e < M * M) {
+                    const int pos = V == kOffFinerSrc ? (nn >> 1) + (nn & 1) * 24 : nn;
+                    T[pos * TROW + mm] = pair_terms_g(fma(double(mm - MMIN), g, u00), fma(double(nn - MMIN), g, v00),
+                                                      lntab_g, tab_idx0, keep);
+                }
             }
         };
 
-        bool any_cur, any_next = false;
+        bool any_cur = false, any_next = false;
         int b_cur = lookup(n0, any_cur), b_next = -1;
         if (any_cur) build(n0, sT);
         __syncthreads();
         for (int n = n0; n < n1; ++n) {
             b_next = lookup(n + 1, any_next);
             if (!any_cur && !any_next) continue;                 // nothing built, nothing consumed: no barrier needed
-            if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * kBlkT);
-            if (have_a && b_cur >= 0) {
-                // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 + 17 + 7]
+            if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * TBUF);
+            if (my_patch >= 0 && b_cur >= 0) {
+                // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
                 const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b_cur) * kPatchQStride);
                 __syncwarp();
 #pragma unroll
@@ -266,26 +296,32 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                     }
                 }
                 __syncwarp();
-                const double2 *T = sT + ((n - n0) & 1) * kBlkT;
-                const int cbase = 8 - k0;
+                const double2 *T = sT + ((n - n0) & 1) * TBUF;
+                if (V == kOffSame) T += (15 - l) * TROW + 8 - 8 * h;
+                else if (V == kOffCoarserSrc) T += (15 - l) * TROW + 1 - h;
+                else T += (15 - l) * TROW + 16 - 16 * h;
 #pragma unroll 1
                 for (int j = 0; j <= P; ++j) {
-                    const double2 *trow = T + (j - l + 15) * kBlkTRow + cbase;
-                    const double *wrow = W + j * kBlkWRow + 1;            // wrow[7 + i] = weight of vertex i
+                    const double2 *trow;
+                    if (V == kOffSame) trow = T + j * TROW;                                  // row j - l + 15
+                    else if (V == kOffCoarserSrc) trow = T + 2 * j * TROW;                   // row 2 j - l + 15
+                    else trow = T + ((j >> 1) + (j & 1) * 24) * TROW;                        // row j - 2 l + 30, stored split
+                    const double *wrow = W + j * kBlkWRow + 8;            // wrow[i] = weight of vertex i
                     double wv[P + 2];                                     // compile-time indices only: registers
 #pragma unroll
-                    for (int t = 0; t < P + kBlkR; ++t) {
+                    for (int t = 0; t < NT; ++t) {
                         if ((t & 1) == 0 && t <= P) {                     // vertices t, t+1 (column 17 is zero padding)
-                            const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t + 7);
+                            const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t);
                             wv[t] = w2.x;
                             wv[t + 1] = w2.y;
                         }
-                        const double2 Tv = trow[t];
+                        const double2 Tv = trow[V == kOffCoarserSrc ? 2 * t : t];
 #pragma unroll
                         for (int r = 0; r < kBlkR; ++r) {
-                            if (t + r >= 7 && t + r <= 7 + P) {      // vertex i = t + r - 7 exists (compile-time)
-                                ax[r] = fma(wv[t + r - 7], Tv.x, ax[r]);
-                                ay[r] = fma(wv[t + r - 7], Tv.y, ay[r]);
+                            const int i = V == kOffFinerSrc ? t + 2 * r - 14 : t + r - 7;     // compile-time
+                            if (i >= 0 && i <= P) {
+                                ax[r] = fma(wv[i], Tv.x, ax[r]);
+                                ay[r] = fma(wv[i], Tv.y, ay[r]);
                             }
                         }
                     }
@@ -294,10 +330,11 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
             __syncthreads();
             b_cur = b_next; any_cur = any_next;
         }
-        if (have_a) {
+        if (my_patch >= 0) {
 #pragma unroll
             for (int r = 0; r < kBlkR; ++r) {
-                const int64_t lt = (int64_t(grp.first + warp) * (P * P) + l * P + k0 + r) - first;
+                const int k = V == kOffCoarserSrc ? 2 * r + h : 8 * h + r;
+                const int64_t lt = (int64_t(my_patch) * (P * P) + l * P + k) - first;
                 if (lt >= 0 && lt < count) {
                     part[(int64_t(sp) * 2 + 0) * count + lt] = ax[r];
                     part[(int64_t(sp) * 2 + 1) * count + lt] = ay[r];
@@ -307,19 +344,39 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     }
 }
 
-size_t patch_offset_smem_bytes() { return size_t(2) * kBlkT * 16 + size_t(kOffWarps) * kBlkW * 8; }
-
-cudaError_t configure_patch_offset() {
-    return cudaFuncSetAttribute(patch_offset_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(patch_offset_smem_bytes()));
+template <int V>
+constexpr size_t patch_offset_smem() {
+    return size_t(2) * (V == kOffSame ? 32 * 33 : kOffTMax) * 16 + size_t(kOffWarps) * kBlkW * 8;
 }
 
-void launch_patch_offset(const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first, int64_t count,
-                         cudaStream_t s) {
-    if (count == 0 || po.n_groups == 0) return;
-    patch_offset_kernel<<<po.grid, kOffWarps * 32, patch_offset_smem_bytes(), s>>>(pa.info, pa.levels, pa.groups, pa.pmap, pa.wQ, d.lntab,
-                                                          d.tab_idx0, po.g_first, po.n_groups, po.n_split, first,
-                                                          count, d.part, d.queue + 1, kLogKeepMask);
+cudaError_t configure_patch_offset() {
+    cudaError_t e = cudaFuncSetAttribute(patch_offset_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         int(patch_offset_smem<0>()));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(patch_offset_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 int(patch_offset_smem<1>()));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(patch_offset_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 int(patch_offset_smem<2>()));
+    return e;
+}
+
+void launch_patch_offset(int V, const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
+                         int64_t count, double *part, cudaStream_t s) {
+    const PatchGroup *groups = pa.groups + (V == kOffCoarserSrc ? po.n_groups0 : 0);
+    const int n_groups = V == kOffCoarserSrc ? po.n_groups1 : po.n_groups0;
+    if (count == 0 || n_groups == 0) return;
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(2) * sms));
+#define SG_LAUNCH_OFFSET(VV)                                                                                          \
+    patch_offset_kernel<VV><<<grid, kOffWarps * 32, patch_offset_smem<VV>(), s>>>(                                    \
+        pa.info, pa.levels, groups, pa.pmap, pa.wQ, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,        \
+        po.last_patch, first, count, part, d.queue + 1 + VV, kLogKeepMask)
+    if (V == kOffSame) SG_LAUNCH_OFFSET(0);
+    else if (V == kOffCoarserSrc) SG_LAUNCH_OFFSET(1);
+    else SG_LAUNCH_OFFSET(2);
+#undef SG_LAUNCH_OFFSET
 }
 
 size_t patch_smem_bytes(int P, int tab_entries) {
@@ -335,16 +392,16 @@ cudaError_t configure_patch_kernels(int P, int tab_entries) {
 }
 
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                              int64_t count, double *part, int skip_same_level, cudaStream_t s) {
+                              int64_t count, double *part, int skip_near, cudaStream_t s) {
     if (count == 0) return;
     if (pa.P == 16)
         patch_interaction_kernel<16><<<pp.grid, 256, pp.smem, s>>>(
             pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
-            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_same_level);
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_near);
     else
         patch_interaction_kernel<8><<<pp.grid, 64, pp.smem, s>>>(
             pa.info, pa.wP, pa.wstride, d.lntab, d.tab_idx0, d.tab_entries, pa.n_patches, pp.patches_per_split,
-            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_same_level);
+            pp.n_split, pp.first_patch, pp.n_tpatches, first, count, part, d.queue, kLogKeepMask, skip_near);
 }
 
 }  // namespace sg

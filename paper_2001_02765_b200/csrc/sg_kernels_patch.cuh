@@ -17,9 +17,17 @@ struct PatchLevel {                   // the leaf patches of one level (contiguo
     int32_t cw;                       // cell width in lattice units
 };
 
-struct PatchGroup {                   // <= 8 consecutive target patches of one level: one CTA work item per split
-    int32_t level, first, n;
-    int32_t dpi_min, ndpi, dpj_min, ndpj;   // box of patch offsets d = B - A that can hit a source patch of the level
+// Pair classes of patch_offset_kernel<V>: source patches of the target's own level (V = 0), of the next coarser
+// level (V = 1) and of the next finer level (V = 2).
+constexpr int kOffSame = 0, kOffCoarserSrc = 1, kOffFinerSrc = 2;
+
+struct PatchGroup {                   // <= 8 target patches of one level (list 1: of one parity class (pi % 2, pj % 2))
+    int32_t level, n;
+    int32_t patch[8];                 // patch indices (unused entries: -1)
+    int32_t pmin, pmax;               // smallest / largest patch index (target-range test)
+    // per pair class: box of patch offsets d that can hit a source patch, in units of the FINER level's patch
+    // size: {dpi_min, ndpi, dpj_min, ndpj}; class 1 steps d by 2 (A + d must be even); ndpi = 0: class absent
+    int32_t box[3][4];
 };
 
 constexpr int kPatchQStride = 17 * 18;   // doubles per patch in wQ
@@ -49,18 +57,19 @@ struct PatchPlan {
 size_t patch_smem_bytes(int P, int tab_entries);
 cudaError_t configure_patch_kernels(int P, int tab_entries);
 void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s);
+// skip_near: 0 = all patch pairs, 1 = skip pairs of the same level, 2 = skip pairs at most one level apart
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
-                              int64_t count, double *part, int skip_same_level, cudaStream_t s);
-// register-blocked same-level kernel with one offset table per CTA (P = 16); uses the second queue counter
-// (d.queue + 1) and writes the first po.n_split slots of d.part
+                              int64_t count, double *part, int skip_near, cudaStream_t s);
+// register-blocked kernels with one offset table per CTA (P = 16), patch pairs at most one level apart
 struct OffsetPlan {
-    int g_first = 0, n_groups = 0;    // groups touched by the target range
+    int n_groups0 = 0, n_groups1 = 0; // group list 0 (pair classes 0 and 2) and list 1 (class 1), stored back to back
     int n_split = 1;                  // splits of every group's offset list
-    int grid = 0;
+    int first_patch = 0, last_patch = -1;   // target patches touched by the target range
+    bool variant[3] = {false, false, false};   // pair classes present in this layout
 };
-size_t patch_offset_smem_bytes();
 cudaError_t configure_patch_offset();
-void launch_patch_offset(const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first, int64_t count,
-                         cudaStream_t s);
+// pair class V writes po.n_split slots of [2][count] partial sums at `part` and uses queue counter 1 + V
+void launch_patch_offset(int V, const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
+                         int64_t count, double *part, cudaStream_t s);
 
 }  // namespace sg
