@@ -125,9 +125,14 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
  *                    is tabulated once on the patch pair's offset lattice and the pairs reduce to 2 FMA each;
  *                    patch pairs more than one level apart are summed directly.  Needs P = 8 or 16
  *                    (SG_ERR_ARG otherwise).  Same sum, same tolerances; the slope path always runs DIRECT.
+ *                    Large P = 16 problems (>= 4 target patches per SM) run the register-blocked kernels that
+ *                    share one offset table per CTA; smaller ones a lighter one-target-per-thread kernel.
+ *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but the register-blocked kernels at any problem size
+ *                    (P = 16 only, SG_ERR_ARG otherwise).  For tests and profiling.
  */
 #define SG_MODE_DIRECT  0
 #define SG_MODE_LATTICE 1
+#define SG_MODE_LATTICE_BLOCKED 2
 int sg_set_interaction_mode(sg_ctx *ctx, int mode);
 
 /* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */

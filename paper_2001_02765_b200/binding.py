@@ -201,8 +201,9 @@ class SgDisk:
         self._first, self._count = int(first), int(count)
 
     def set_interaction_mode(self, mode: str):
-        """'direct' (every pair: sqrt + 2 ln) or 'lattice' (per-patch-pair offset tables; P = 8 or 16)."""
-        self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1}[mode]))
+        """'direct' (every pair: sqrt + 2 ln), 'lattice' (per-patch-pair offset tables; P = 8 or 16) or
+        'lattice_blocked' (the register-blocked offset-table kernels at any size; P = 16)."""
+        self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1, "lattice_blocked": 2}[mode]))
 
     def force(self, Fx=None, Fy=None):
         """Fx, Fy (CUDA float64 [count]) at the leaf centres of the current target range."""

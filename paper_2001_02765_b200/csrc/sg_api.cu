@@ -25,6 +25,7 @@ struct sg_ctx {
     std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning): list 0 then list 1
     int patch_n_groups0 = 0;                // groups of list 0 (pair classes "same level", "finer source")
     bool use_patch = false;      // sg_set_interaction_mode
+    bool force_blocked = false;  // SG_MODE_LATTICE_BLOCKED
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
@@ -149,6 +150,11 @@ OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
     const int slots = c->sm_count * 2;
     po.n_split = std::max(1, std::min(64, (6 * slots + touched - 1) / std::max(1, touched)));
     return po;
+}
+
+// small problems: more, lighter CTAs (generic kernel) unless the caller insists on the blocked kernels
+bool use_blocked(const sg_ctx *c, const PatchPlan &pp) {
+    return c->patch.blocked && (c->force_blocked || pp.n_tpatches >= 4 * c->sm_count);
 }
 
 int upload_patches(sg_ctx *c) {
@@ -452,7 +458,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     bool blocked = false, far = true;
     if (by_patch) {
         pp = make_patch_plan(c);
-        blocked = c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count;   // small problems: more, lighter CTAs
+        blocked = use_blocked(c, pp);
         if (blocked) {
             po = make_offset_plan(c, pp);
             far = c->host.n_levels > 2;
@@ -491,11 +497,18 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
 
 int sg_set_interaction_mode(sg_ctx *c, int mode) {
     if (!c) return SG_ERR_ARG;
-    if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE) { c->err = "unknown interaction mode"; return SG_ERR_ARG; }
+    if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE && mode != SG_MODE_LATTICE_BLOCKED) {
+        c->err = "unknown interaction mode"; return SG_ERR_ARG;
+    }
     if (mode == SG_MODE_LATTICE && c->host.P != 8 && c->host.P != 16) {
         c->err = "SG_MODE_LATTICE needs patches of 8 x 8 or 16 x 16 cells"; return SG_ERR_ARG;
     }
-    c->use_patch = mode == SG_MODE_LATTICE;
+    if (mode == SG_MODE_LATTICE_BLOCKED && (c->host.P != 16 || (c->device >= 0 && !c->patch.blocked))) {
+        c->err = "SG_MODE_LATTICE_BLOCKED needs patches of 16 x 16 cells (and per-level patch maps that fit)";
+        return SG_ERR_ARG;
+    }
+    c->use_patch = mode != SG_MODE_DIRECT;
+    c->force_blocked = mode == SG_MODE_LATTICE_BLOCKED;
     return SG_OK;
 }
 
@@ -516,7 +529,7 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
         int n = 1;
         if (c->use_patch && !c->linear && c->count > 0) {
             const PatchPlan pp = make_patch_plan(c);
-            if (c->patch.blocked && pp.n_tpatches >= 4 * c->sm_count) {
+            if (use_blocked(c, pp)) {
                 const OffsetPlan po = make_offset_plan(c, pp);
                 n = int(po.variant[0]) + int(po.variant[1]) + int(po.variant[2]) + (c->host.n_levels > 2 ? 1 : 0);
             }

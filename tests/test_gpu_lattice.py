@@ -6,7 +6,8 @@ import numpy as np
 import pytest
 
 import oracle
-from workloads import Layout, make_config, cell_rects, sample_targets, paper_ilr_layout, nested_layout, kuzmin_sigma
+from workloads import (Layout, make_config, cell_rects, sample_targets, paper_ilr_layout, nested_layout, kuzmin_sigma,
+                       random_refined_layout)
 from workloads.configs import cell_centres
 
 pytestmark = pytest.mark.gpu
@@ -102,6 +103,49 @@ def test_five_nested_levels_small_patches(torch_cuda):
     check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
 
 
+def _noisy_kuzmin(lay, seed, a=0.3):
+    x, y, _ = cell_centres(lay)
+    return kuzmin_sigma(x, y, a=a) * (1 + 0.2 * np.random.default_rng(seed).uniform(-1, 1, lay.n_cells))
+
+
+def test_blocked_kernels_four_nested_levels(torch_cuda):
+    """P = 16, four nested levels, ALL targets vs the oracle with the register-blocked offset-table kernels forced
+    (SG_MODE_LATTICE_BLOCKED): same-level, coarser-source and finer-source classes plus the direct far pairs."""
+    lay = nested_layout(4, 64, 8.0, 16)
+    sigma = _noisy_kuzmin(lay, 21)
+    gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice_blocked")
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_blocked_kernels_irregular_hierarchy(torch_cuda, seed):
+    """Ragged, unbalanced three-level hierarchy with holes (groups with fewer than 8 patches, patches of every parity,
+    offsets without a source patch): all targets vs the oracle, agreement with the direct kernel, target slices."""
+    lay = random_refined_layout(seed, 6, 16, 3, 0.3)
+    sigma = _noisy_kuzmin(lay, 30 + seed)
+    gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice_blocked")
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+    dx, dy = gpu_force(torch_cuda, lay, sigma, "direct")
+    s = max(np.abs(dx).max(), np.abs(dy).max())
+    assert max(np.abs(gx - dx).max(), np.abs(gy - dy).max()) <= 1e-12 * s
+    n = lay.n_cells
+    for first, count in ((0, 1), (300, n // 2), (n // 2 + 77, n - n // 2 - 77), (n - 1, 1), (255, 2), (5, 0)):
+        rx, ry = gpu_force(torch_cuda, lay, sigma, "lattice_blocked", target_range=(first, count))
+        assert rx.shape == (count,)
+        if count:
+            assert np.array_equal(rx, gx[first:first + count]) and np.array_equal(ry, gy[first:first + count])
+
+
+def test_blocked_kernels_single_level_and_single_patch(torch_cuda):
+    lay, sigma = make_config(1)                                    # 16 patches, one level
+    gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice_blocked")
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+    one = Layout(1, np.array([0.125]), -1.0, -1.0, 16, np.array([[0, 0, 0]], dtype=np.int32))
+    sigma1 = np.random.default_rng(5).uniform(0.5, 1.5, one.n_cells)
+    gx, gy = gpu_force(torch_cuda, one, sigma1, "lattice_blocked")
+    check(gx, gy, *oracle_force(one, sigma1, np.arange(one.n_cells)))
+
+
 def test_unsupported_patch_size_is_refused(torch_cuda):
     from paper_2001_02765_b200 import SgDisk, SgError, binding
     lay = paper_ilr_layout(32, 2)                                  # P = 1 quadtree
@@ -110,3 +154,9 @@ def test_unsupported_patch_size_is_refused(torch_cuda):
             d.set_interaction_mode("lattice")
         assert e.value.code == binding.SG_ERR_ARG
         d.set_interaction_mode("direct")
+    lay2, _ = make_config(2)                                       # P = 8: generic lattice kernel only
+    with SgDisk.from_layout(lay2, device=0) as d:
+        d.set_interaction_mode("lattice")
+        with pytest.raises(SgError) as e:
+            d.set_interaction_mode("lattice_blocked")
+        assert e.value.code == binding.SG_ERR_ARG

@@ -154,6 +154,24 @@ def nested_layout(n_levels: int, n: int, half_extent: float, P: int) -> Layout:
                   _sorted_patches(rows))
 
 
+def random_refined_layout(seed: int, n0: int, P: int, n_levels: int, frac: float, half_extent: float = 1.0) -> Layout:
+    """Irregular hierarchy for edge-case tests: an n0 x n0-patch base grid; on every level a seeded random fraction
+    `frac` of the leaf patches is replaced by its four children.  No 2:1 balancing, ragged level shapes, patches of
+    every parity, levels with holes."""
+    rng = np.random.default_rng(seed)
+    leaves = [(0, i * P, j * P) for j in range(n0) for i in range(n0)]
+    for l in range(n_levels - 1):
+        nxt = []
+        for (lv, i0, j0) in leaves:
+            if lv == l and rng.uniform() < frac:
+                nxt += [(l + 1, 2 * i0 + a * P, 2 * j0 + b * P) for b in (0, 1) for a in (0, 1)]
+            else:
+                nxt.append((lv, i0, j0))
+        leaves = nxt
+    h0 = 2.0 * half_extent / (n0 * P)
+    return Layout(n_levels, h0 / 2.0 ** np.arange(n_levels), -half_extent, -half_extent, P, _sorted_patches(leaves))
+
+
 def _cfg2_layout() -> Layout:
     rows = []
     for j in range(0, 64, 8):
