@@ -23,7 +23,7 @@ struct sg_ctx {
     LinArrays lin;
     PatchArrays patch;           // lattice-offset reuse path (P = 8 or 16)
     std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning): list 0 then list 1
-    int patch_n_groups0 = 0;                // groups of list 0 (pair classes "same level", "finer source")
+    int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
     bool use_patch = false;      // sg_set_interaction_mode
     bool force_blocked = false;  // SG_MODE_LATTICE_BLOCKED
     int64_t first = 0, count = 0;
@@ -136,20 +136,25 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
 OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
     OffsetPlan po;
     if (c->count == 0) return po;
-    po.n_groups0 = c->patch_n_groups0;
-    po.n_groups1 = int(c->patch_groups.size()) - po.n_groups0;
+    for (int q = 0; q < 3; ++q) po.n_groups[q] = c->patch_n_groups[q];
     po.first_patch = pp.first_patch;
     po.last_patch = pp.first_patch + pp.n_tpatches - 1;
     int touched = 0;
     for (size_t i = 0; i < c->patch_groups.size(); ++i) {
         const PatchGroup &g = c->patch_groups[i];
         if (g.pmax < po.first_patch || g.pmin > po.last_patch) continue;
-        if (int(i) < po.n_groups0) ++touched;
-        for (int v = 0; v < 3; ++v) po.variant[v] = po.variant[v] || g.box[v][1] > 0;
+        if (int(i) < po.n_groups[0]) ++touched;
+        for (int v = 0; v < kOffClasses; ++v) po.variant[v] = po.variant[v] || g.box[v][1] > 0;
     }
     const int slots = c->sm_count * 2;
     po.n_split = std::max(1, std::min(64, (6 * slots + touched - 1) / std::max(1, touched)));
     return po;
+}
+
+int offset_classes(const OffsetPlan &po) {
+    int n = 0;
+    for (int v = 0; v < kOffClasses; ++v) n += int(po.variant[v]);
+    return n;
 }
 
 // small problems: more, lighter CTAs (generic kernel) unless the caller insists on the blocked kernels
@@ -203,63 +208,72 @@ int upload_patches(sg_ctx *c) {
             p = q;
         }
         // groups of 8 target patches in sorted order with their offset boxes.  List 0 (any patches of a level) serves
-        // the pair classes "same level" and "finer source"; list 1 (patches of one parity class (pi % 2, pj % 2))
-        // serves "coarser source", where A + d must be even for the whole group.
-        std::vector<PatchGroup> glist[2];
+        // the pair classes "same level" and "finer source"; lists 1 / 2 (patches of one residue class of (pi, pj)
+        // mod F = 2 / 4) serve the sources F times coarser, where A + d must be a multiple of F for the whole group.
+        std::vector<PatchGroup> glist[3];
+        auto level_ok = [&](int L) { return L >= 0 && L < h.n_levels && lev[size_t(L)].n > 0; };
         for (int L = 0; L < h.n_levels && ok; ++L) {
             const PatchLevel &l = lev[size_t(L)];
             if (l.n == 0) continue;
-            for (int cls = -1; cls < 4; ++cls) {                       // -1: list 0
-                if (cls >= 0 && (L == 0 || lev[size_t(L - 1)].n == 0)) break;
-                std::vector<int32_t> members;
-                for (int32_t r = l.p0; r < l.p0 + l.n; ++r)
-                    if (cls < 0 || (((h.patches[size_t(r)].i0 / h.P) & 1) == (cls & 1) && ((h.patches[size_t(r)].j0 / h.P) & 1) == (cls >> 1)))
-                        members.push_back(r);
-                for (size_t m0 = 0; m0 < members.size() && ok; m0 += 8) {
-                    PatchGroup gr;
-                    std::memset(&gr, 0, sizeof gr);
-                    gr.level = L;
-                    gr.n = int(std::min<size_t>(8, members.size() - m0));
-                    int gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
-                    gr.pmin = INT32_MAX; gr.pmax = INT32_MIN;
-                    for (int w = 0; w < 8; ++w) {
-                        gr.patch[w] = w < gr.n ? members[m0 + size_t(w)] : -1;
-                        if (w >= gr.n) continue;
-                        const sg_patch &q = h.patches[size_t(gr.patch[w])];
-                        gimin = std::min(gimin, q.i0 / h.P); gimax = std::max(gimax, q.i0 / h.P);
-                        gjmin = std::min(gjmin, q.j0 / h.P); gjmax = std::max(gjmax, q.j0 / h.P);
-                        gr.pmin = std::min(gr.pmin, gr.patch[w]); gr.pmax = std::max(gr.pmax, gr.patch[w]);
-                    }
-                    // d ranges over [lo, hi] per axis; the coarser-source class keeps the parity of the patch positions
-                    auto set_box = [&](int v, int64_t lox, int64_t hix, int64_t loy, int64_t hiy, int step) {
-                        if (step == 2) {
-                            if ((lox & 1) != (cls & 1)) ++lox;
-                            if ((loy & 1) != (cls >> 1)) ++loy;
+            for (int list = 0; list < 3 && ok; ++list) {
+                const int F = 1 << list;                                // residue classes mod F
+                if (list > 0 && !level_ok(L - list)) continue;
+                for (int cls = 0; cls < F * F && ok; ++cls) {
+                    const int cx = cls % F, cy = cls / F;
+                    std::vector<int32_t> members;
+                    for (int32_t r = l.p0; r < l.p0 + l.n; ++r)
+                        if ((h.patches[size_t(r)].i0 / h.P) % F == cx && (h.patches[size_t(r)].j0 / h.P) % F == cy)
+                            members.push_back(r);
+                    for (size_t m0 = 0; m0 < members.size() && ok; m0 += 8) {
+                        PatchGroup gr;
+                        std::memset(&gr, 0, sizeof gr);
+                        gr.level = L;
+                        gr.n = int(std::min<size_t>(8, members.size() - m0));
+                        int64_t gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
+                        gr.pmin = INT32_MAX; gr.pmax = INT32_MIN;
+                        for (int w = 0; w < 8; ++w) {
+                            gr.patch[w] = w < gr.n ? members[m0 + size_t(w)] : -1;
+                            if (w >= gr.n) continue;
+                            const sg_patch &q = h.patches[size_t(gr.patch[w])];
+                            gimin = std::min<int64_t>(gimin, q.i0 / h.P); gimax = std::max<int64_t>(gimax, q.i0 / h.P);
+                            gjmin = std::min<int64_t>(gjmin, q.j0 / h.P); gjmax = std::max<int64_t>(gjmax, q.j0 / h.P);
+                            gr.pmin = std::min(gr.pmin, gr.patch[w]); gr.pmax = std::max(gr.pmax, gr.patch[w]);
                         }
-                        const int64_t nx = hix >= lox ? (hix - lox) / step + 1 : 0, ny = hiy >= loy ? (hiy - loy) / step + 1 : 0;
-                        if (nx * ny > (int64_t(1) << 30)) { ok = false; return; }
-                        gr.box[v][0] = int32_t(lox); gr.box[v][1] = int32_t(nx * ny > 0 ? nx : 0);
-                        gr.box[v][2] = int32_t(loy); gr.box[v][3] = int32_t(nx * ny > 0 ? ny : 0);
-                    };
-                    if (cls < 0) {
-                        set_box(kOffSame, l.pimin - gimax, l.pimin + l.npx - 1 - gimin, l.pjmin - gjmax, l.pjmin + l.npy - 1 - gjmin, 1);
-                        if (L + 1 < h.n_levels && lev[size_t(L + 1)].n > 0) {   // 2 A + d inside the finer level's box
-                            const PatchLevel &f0 = lev[size_t(L + 1)];
-                            set_box(kOffFinerSrc, int64_t(f0.pimin) - 2 * int64_t(gimax), int64_t(f0.pimin + f0.npx - 1) - 2 * int64_t(gimin),
-                                    int64_t(f0.pjmin) - 2 * int64_t(gjmax), int64_t(f0.pjmin + f0.npy - 1) - 2 * int64_t(gjmin), 1);
+                        // d ranges over [lo, hi] per axis in steps of `step`, starting where A + d is a multiple of it
+                        auto set_box = [&](int v, int64_t lox, int64_t hix, int64_t loy, int64_t hiy, int step) {
+                            while (((lox + cx) % step + step) % step != 0) ++lox;
+                            while (((loy + cy) % step + step) % step != 0) ++loy;
+                            const int64_t nx = hix >= lox ? (hix - lox) / step + 1 : 0, ny = hiy >= loy ? (hiy - loy) / step + 1 : 0;
+                            if (nx * ny > (int64_t(1) << 30)) { ok = false; return; }
+                            gr.box[v][0] = int32_t(lox); gr.box[v][1] = int32_t(nx * ny > 0 ? nx : 0);
+                            gr.box[v][2] = int32_t(loy); gr.box[v][3] = int32_t(nx * ny > 0 ? ny : 0);
+                        };
+                        auto hi_i = [](const PatchLevel &q) { return int64_t(q.pimin) + q.npx - 1; };
+                        auto hi_j = [](const PatchLevel &q) { return int64_t(q.pjmin) + q.npy - 1; };
+                        if (list == 0) {
+                            set_box(kOffSame, l.pimin - gimax, hi_i(l) - gimin, l.pjmin - gjmax, hi_j(l) - gjmin, 1);
+                            for (int dl = 1; dl <= 2; ++dl) {            // source patch F A + d inside the finer level's box
+                                if (!level_ok(L + dl)) continue;
+                                const PatchLevel &f0 = lev[size_t(L + dl)];
+                                const int64_t Ff = 1 << dl;
+                                set_box(dl == 1 ? kOffFinerSrc : kOffFinerSrc4, f0.pimin - Ff * gimax, hi_i(f0) - Ff * gimin,
+                                        f0.pjmin - Ff * gjmax, hi_j(f0) - Ff * gjmin, 1);
+                            }
+                        } else {                                         // source patch (A + d) / F inside the coarser level's box
+                            const PatchLevel &c0 = lev[size_t(L - list)];
+                            set_box(list == 1 ? kOffCoarserSrc : kOffCoarserSrc4, F * int64_t(c0.pimin) - gimax, F * hi_i(c0) - gimin,
+                                    F * int64_t(c0.pjmin) - gjmax, F * hi_j(c0) - gjmin, F);
                         }
-                    } else {                                           // (A + d) / 2 inside the coarser level's box
-                        const PatchLevel &c0 = lev[size_t(L - 1)];
-                        set_box(kOffCoarserSrc, 2 * int64_t(c0.pimin) - gimax, 2 * int64_t(c0.pimin + c0.npx - 1) - gimin,
-                                2 * int64_t(c0.pjmin) - gjmax, 2 * int64_t(c0.pjmin + c0.npy - 1) - gjmin, 2);
+                        glist[list].push_back(gr);
                     }
-                    glist[cls < 0 ? 0 : 1].push_back(gr);
                 }
             }
         }
-        groups = glist[0];
-        c->patch_n_groups0 = int(glist[0].size());
-        groups.insert(groups.end(), glist[1].begin(), glist[1].end());
+        groups.clear();
+        for (int list = 0; list < 3; ++list) {
+            c->patch_n_groups[list] = int(glist[list].size());
+            groups.insert(groups.end(), glist[list].begin(), glist[list].end());
+        }
         if (ok) {
             if ((rc = upload(c, &pa.levels, lev)) || (rc = upload(c, &pa.groups, groups)) || (rc = upload(c, &pa.pmap, pmap)))
                 return rc;
@@ -461,9 +475,8 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
         blocked = use_blocked(c, pp);
         if (blocked) {
             po = make_offset_plan(c, pp);
-            far = c->host.n_levels > 2;
-            const int nv = int(po.variant[0]) + int(po.variant[1]) + int(po.variant[2]);
-            p.n_split = nv * po.n_split + (far ? pp.n_split : 0);  // finalise adds p.n_split partial sums per target
+            far = c->host.n_levels > 3;
+            p.n_split = offset_classes(po) * po.n_split + (far ? pp.n_split : 0);  // finalise adds p.n_split partial sums per target
         } else {
             p.n_split = pp.n_split;
         }
@@ -476,13 +489,13 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     else if (by_patch) {
         double *part = c->dev.part;        // every launch writes its own n_split slots of [2][count] partial sums
         if (blocked)
-            for (int v = 0; v < 3; ++v)
+            for (int v = 0; v < kOffClasses; ++v)
                 if (po.variant[v]) {
                     launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, s);
                     part += int64_t(po.n_split) * 2 * c->count;
                 }
         if (!blocked || far)
-            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 2 : 0, s);
+            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 3 : 0, s);
     }
     else launch_interaction(c->dev, p, s);
     if (c->timing) {
@@ -531,7 +544,7 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
             const PatchPlan pp = make_patch_plan(c);
             if (use_blocked(c, pp)) {
                 const OffsetPlan po = make_offset_plan(c, pp);
-                n = int(po.variant[0]) + int(po.variant[1]) + int(po.variant[2]) + (c->host.n_levels > 2 ? 1 : 0);
+                n = offset_classes(po) + (c->host.n_levels > 3 ? 1 : 0);
             }
         }
         *force_launches = c->count > 0 ? n + 1 : 0;

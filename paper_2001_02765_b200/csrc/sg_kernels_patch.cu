@@ -164,7 +164,6 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 // Every per-patch sum stays in one accumulator chain (split chains cancel badly).
 // ------------------------------------------------------------------------------------------------
 constexpr int kOffWarps = 8, kBlkR = 8, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
-constexpr int kOffTRowMax = 49, kOffTMax = 48 * kOffTRowMax;            // largest table: V = 1, 48 x 48 entries
 
 __device__ __forceinline__ double fast_ln_g(double a, const double *__restrict__ lntab_g, int tab_idx0, uint32_t keep) {
     const uint32_t hi = uint32_t(__double2hiint(a));
@@ -190,23 +189,40 @@ __device__ __forceinline__ double2 pair_terms_g(double u, double v, const double
                         flip_sign_by(fast_ln_g(fabs(u) + r, lntab_g, tab_idx0, keep), u));
 }
 
+// compile-time description of pair class V (kOffSame, kOffCoarserSrc, kOffFinerSrc, kOffCoarserSrc4, kOffFinerSrc4)
 template <int V>
-__global__ void __launch_bounds__(kOffWarps * 32, 2)
+struct OffCls {
+    static constexpr int P = 16;
+    static constexpr bool coarser = V == kOffCoarserSrc || V == kOffCoarserSrc4, finer = V == kOffFinerSrc || V == kOffFinerSrc4;
+    static constexpr int F = V == kOffSame ? 1 : (V == kOffCoarserSrc || V == kOffFinerSrc) ? 2 : 4;   // pitch ratio
+    static constexpr int RA = finer ? F : 1, RB = coarser ? F : 1;        // target / source pitch in units of g
+    static constexpr int M = P * RB + (P - 1) * RA + 1, MMIN = (P - 1) * RA;      // table side 32, 48, 47, 80, 77
+    static constexpr int RPC = (M + RA - 1) / RA;                         // stored rows per row class (finer source)
+    static constexpr int ROWS = RA * RPC, TROW = (M | 1) == M ? M + 2 : M + 1;    // odd pitch >= M + 1
+    static constexpr int TBUF = ROWS * TROW;
+    static constexpr bool DB = F < 4;                                     // double-buffered tables (two CTAs per SM)
+    static constexpr int LDIST = coarser ? -(F == 2 ? 1 : 2) : finer ? (F == 2 ? 1 : 2) : 0;   // source level - target level
+    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16 + size_t(kOffWarps) * kBlkW * 8;
+};
+
+template <int V>
+__global__ void __launch_bounds__(kOffWarps * 32, (OffCls<V>::DB ? 2 : 1))
 patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
                     const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int n_groups,
                     int n_split, int first_patch, int last_patch, int64_t first, int64_t count,
                     double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
-    constexpr int P = 16;
-    constexpr int RA = V == kOffFinerSrc ? 2 : 1, RB = V == kOffCoarserSrc ? 2 : 1;
-    constexpr int M = P * RB + (P - 1) * RA + 1, MMIN = (P - 1) * RA;     // table side: 32, 48, 47
-    constexpr int TROW = V == kOffSame ? 33 : kOffTRowMax, TBUF = V == kOffSame ? 32 * 33 : kOffTMax;
-    constexpr int STEP = V == kOffCoarserSrc ? 2 : 1;                     // offsets keep A + d even for V = 1
+    using C = OffCls<V>;
+    constexpr int P = 16, F = C::F, M = C::M, MMIN = C::MMIN, TROW = C::TROW, TBUF = C::TBUF;
+    constexpr int STEP = C::coarser ? F : 1;                              // offsets keep A + d a multiple of F
     constexpr int EVALS = (M * M + kOffWarps * 32 - 1) / (kOffWarps * 32);
-    constexpr int NT = V == kOffFinerSrc ? P + 2 * (kBlkR - 1) + 1 : P + kBlkR;   // table entries per thread and row
+    // per thread and source row: coarser source: NCLS column classes of MT targets each, NT table steps;
+    // otherwise 8 consecutive targets, NT table entries
+    constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
+    constexpr int NT = C::finer ? P + F * (kBlkR - 1) + 1 : P + MT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2][TBUF] offset tables, double-buffered
-    double *sW = reinterpret_cast<double *>(sT + 2 * TBUF);                // [warp][17][8 | 18 | 6] weights of B_w
+    double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2 or 1][TBUF] offset tables
+    double *sW = reinterpret_cast<double *>(sT + (C::DB ? 2 : 1) * TBUF);  // [warp][17][8 | 18 | 6] weights of B_w
     __shared__ int s_item;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int l = lane & 15, h = lane >> 4;
@@ -226,14 +242,13 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         if (gp->pmax < first_patch || gp->pmin > last_patch) continue;          // no target of the range in this group
         const int grp_n = gp->n, grp_level = gp->level;
         const PatchLevel lev = levels[grp_level];
-        const int src_level = grp_level + (V == kOffCoarserSrc ? -1 : V == kOffFinerSrc ? 1 : 0);
         const int dpi_min = gp->box[V][0], ndpi = gp->box[V][1], dpj_min = gp->box[V][2], ndpj = gp->box[V][3];
         const int n_off = ndpi * ndpj, per = (n_off + n_split - 1) / n_split;   // 0 when the class is absent here
         const int n0 = sp * per, n1 = min(n_off, n0 + per);
-        const PatchLevel slev = levels[n_off > 0 ? src_level : grp_level];
+        const PatchLevel slev = levels[n_off > 0 ? grp_level + C::LDIST : grp_level];
         const double g = double(min(lev.cw, slev.cw));
 
-        // lane w < grp.n of every warp holds the patch position of target patch A_w (for the map look-ups)
+        // lane w < grp_n of every warp holds the patch position of target patch A_w (for the map look-ups)
         int api = 0, apj = 0;
         if (lane < grp_n) {
             const PatchInfo A = info[gp->patch[lane]];
@@ -251,89 +266,102 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
             if (n < n1 && lane < grp_n) {
                 const int dx = dpi_min + STEP * (n % ndpi), dy = dpj_min + STEP * (n / ndpi);
                 int bi, bj;
-                if (V == kOffSame) { bi = api + dx; bj = apj + dy; }
-                else if (V == kOffCoarserSrc) { bi = (api + dx) >> 1; bj = (apj + dy) >> 1; }
-                else { bi = 2 * api + dx; bj = 2 * apj + dy; }
+                if (C::coarser) { bi = (api + dx) / F; bj = (apj + dy) / F; }     // exact: A + d is a multiple of F
+                else { bi = F * api + dx; bj = F * apj + dy; }
                 bi -= slev.pimin; bj -= slev.pjmin;
                 if (bi >= 0 && bi < slev.npx && bj >= 0 && bj < slev.npy) b = pmap[slev.map_off + bj * slev.npx + bi];
             }
             any = __ballot_sync(0xffffffffu, b >= 0) != 0u;
             return __shfl_sync(0xffffffffu, b, warp & 7);
         };
-        // T[row][col] = pair function at u = B.X0 - x_centre(A, k = 0) + (col - MMIN) g, likewise v
+        // T[row][col] = pair function at u = B.X0 - x_centre(A, k = 0) + (col - MMIN) g, likewise v; for a finer
+        // source the rows are stored by row class (row % RA): the 16 lanes of a half-warp read consecutive stored rows
         auto build = [&](int n, double2 *T) {
             const double u00 = double((dpi_min + STEP * (n % ndpi)) * P) * g - 0.5 * double(lev.cw);
             const double v00 = double((dpj_min + STEP * (n / ndpi)) * P) * g - 0.5 * double(lev.cw);
-#pragma unroll
+#pragma unroll 4
             for (int q = 0; q < EVALS; ++q) {
                 const int e = tid + q * (kOffWarps * 32), mm = e % M, nn = e / M;
                 if (M * M % (kOffWarps * 32) == 0 || e < M * M) {
-                    const int pos = V == kOffFinerSrc ? (nn >> 1) + (nn & 1) * 24 : nn;
+                    const int pos = nn / C::RA + (nn % C::RA) * C::RPC;
                     T[pos * TROW + mm] = pair_terms_g(fma(double(mm - MMIN), g, u00), fma(double(nn - MMIN), g, v00),
                                                       lntab_g, tab_idx0, keep);
+                }
+            }
+        };
+        auto consume = [&](int b, const double2 *T) {
+            // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
+            const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride);
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                const int e2 = lane + 32 * q;
+                if (e2 < 17 * 9) {
+                    const int j = e2 / 9, c2 = e2 - 9 * j;
+                    *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
+                }
+            }
+            __syncwarp();
+            // entry (row, col) = (j RB - l RA + MMIN, i RB - k RA + MMIN) for vertex (i, j) and target (k, l)
+            if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;   // column F t + this - cc
+            else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
+#pragma unroll 1
+            for (int j = 0; j <= P; ++j) {
+                const double2 *trow = C::coarser ? T + F * j * TROW                                   // row F j - l + 15
+                                                 : T + (j / C::RA + (j % C::RA) * C::RPC) * TROW;      // row j - RA l + MMIN
+                const double *wrow = W + j * kBlkWRow + 8;                // wrow[i] = weight of vertex i
+                double wv[P + 2];                                         // compile-time indices only: registers
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                    if ((t & 1) == 0 && t <= P) {                         // vertices t, t+1 (column 17 is zero padding)
+                        const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t);
+                        wv[t] = w2.x;
+                        wv[t + 1] = w2.y;
+                    }
+#pragma unroll
+                    for (int cc = 0; cc < NCLS; ++cc) {
+                        const double2 Tv = trow[C::coarser ? F * t - cc : t];
+#pragma unroll
+                        for (int m = 0; m < MT; ++m) {
+                            const int i = C::finer ? t + F * m - F * (kBlkR - 1) : t + m - (MT - 1);    // compile-time
+                            if (i >= 0 && i <= P) {
+                                ax[cc * MT + m] = fma(wv[i], Tv.x, ax[cc * MT + m]);
+                                ay[cc * MT + m] = fma(wv[i], Tv.y, ay[cc * MT + m]);
+                            }
+                        }
+                    }
                 }
             }
         };
 
         bool any_cur = false, any_next = false;
         int b_cur = lookup(n0, any_cur), b_next = -1;
-        if (any_cur) build(n0, sT);
-        __syncthreads();
-        for (int n = n0; n < n1; ++n) {
-            b_next = lookup(n + 1, any_next);
-            if (!any_cur && !any_next) continue;                 // nothing built, nothing consumed: no barrier needed
-            if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * TBUF);
-            if (my_patch >= 0 && b_cur >= 0) {
-                // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
-                const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b_cur) * kPatchQStride);
-                __syncwarp();
-#pragma unroll
-                for (int q = 0; q < 5; ++q) {
-                    const int e2 = lane + 32 * q;
-                    if (e2 < 17 * 9) {
-                        const int j = e2 / 9, c2 = e2 - 9 * j;
-                        *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
-                    }
-                }
-                __syncwarp();
-                const double2 *T = sT + ((n - n0) & 1) * TBUF;
-                if (V == kOffSame) T += (15 - l) * TROW + 8 - 8 * h;
-                else if (V == kOffCoarserSrc) T += (15 - l) * TROW + 1 - h;
-                else T += (15 - l) * TROW + 16 - 16 * h;
-#pragma unroll 1
-                for (int j = 0; j <= P; ++j) {
-                    const double2 *trow;
-                    if (V == kOffSame) trow = T + j * TROW;                                  // row j - l + 15
-                    else if (V == kOffCoarserSrc) trow = T + 2 * j * TROW;                   // row 2 j - l + 15
-                    else trow = T + ((j >> 1) + (j & 1) * 24) * TROW;                        // row j - 2 l + 30, stored split
-                    const double *wrow = W + j * kBlkWRow + 8;            // wrow[i] = weight of vertex i
-                    double wv[P + 2];                                     // compile-time indices only: registers
-#pragma unroll
-                    for (int t = 0; t < NT; ++t) {
-                        if ((t & 1) == 0 && t <= P) {                     // vertices t, t+1 (column 17 is zero padding)
-                            const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t);
-                            wv[t] = w2.x;
-                            wv[t + 1] = w2.y;
-                        }
-                        const double2 Tv = trow[V == kOffCoarserSrc ? 2 * t : t];
-#pragma unroll
-                        for (int r = 0; r < kBlkR; ++r) {
-                            const int i = V == kOffFinerSrc ? t + 2 * r - 14 : t + r - 7;     // compile-time
-                            if (i >= 0 && i <= P) {
-                                ax[r] = fma(wv[i], Tv.x, ax[r]);
-                                ay[r] = fma(wv[i], Tv.y, ay[r]);
-                            }
-                        }
-                    }
-                }
-            }
+        if (C::DB) {
+            if (any_cur) build(n0, sT);
             __syncthreads();
-            b_cur = b_next; any_cur = any_next;
+            for (int n = n0; n < n1; ++n) {
+                b_next = lookup(n + 1, any_next);
+                if (!any_cur && !any_next) continue;             // nothing built, nothing consumed: no barrier needed
+                if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * TBUF);
+                if (my_patch >= 0 && b_cur >= 0) consume(b_cur, sT + ((n - n0) & 1) * TBUF);
+                __syncthreads();
+                b_cur = b_next; any_cur = any_next;
+            }
+        } else {                                                 // one table buffer: build, barrier, consume, barrier
+            for (int n = n0; n < n1; ++n) {
+                if (any_cur) {
+                    build(n, sT);
+                    __syncthreads();
+                    if (my_patch >= 0 && b_cur >= 0) consume(b_cur, sT);
+                    __syncthreads();
+                }
+                b_cur = lookup(n + 1, any_cur);
+            }
         }
         if (my_patch >= 0) {
 #pragma unroll
             for (int r = 0; r < kBlkR; ++r) {
-                const int k = V == kOffCoarserSrc ? 2 * r + h : 8 * h + r;
+                const int k = C::coarser ? F * (r % MT) + NCLS * h + r / MT : 8 * h + r;
                 const int64_t lt = (int64_t(my_patch) * (P * P) + l * P + k) - first;
                 if (lt >= 0 && lt < count) {
                     part[(int64_t(sp) * 2 + 0) * count + lt] = ax[r];
@@ -345,38 +373,46 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
 }
 
 template <int V>
-constexpr size_t patch_offset_smem() {
-    return size_t(2) * (V == kOffSame ? 32 * 33 : kOffTMax) * 16 + size_t(kOffWarps) * kBlkW * 8;
+cudaError_t configure_patch_offset_one() {
+    return cudaFuncSetAttribute(patch_offset_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(OffCls<V>::smem));
 }
 
 cudaError_t configure_patch_offset() {
-    cudaError_t e = cudaFuncSetAttribute(patch_offset_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         int(patch_offset_smem<0>()));
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(patch_offset_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 int(patch_offset_smem<1>()));
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(patch_offset_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 int(patch_offset_smem<2>()));
+    cudaError_t e = configure_patch_offset_one<0>();
+    if (e == cudaSuccess) e = configure_patch_offset_one<1>();
+    if (e == cudaSuccess) e = configure_patch_offset_one<2>();
+    if (e == cudaSuccess) e = configure_patch_offset_one<3>();
+    if (e == cudaSuccess) e = configure_patch_offset_one<4>();
     return e;
+}
+
+template <int V>
+void launch_patch_offset_one(const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
+                             int64_t count, double *part, int sms, cudaStream_t s) {
+    const int list = offset_group_list(V);
+    const int n_groups = po.n_groups[list];
+    if (n_groups == 0) return;
+    const PatchGroup *groups = pa.groups;
+    for (int q = 0; q < list; ++q) groups += po.n_groups[q];
+    const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(OffCls<V>::DB ? 2 : 1) * sms));
+    patch_offset_kernel<V><<<grid, kOffWarps * 32, OffCls<V>::smem, s>>>(
+        pa.info, pa.levels, groups, pa.pmap, pa.wQ, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,
+        po.last_patch, first, count, part, d.queue + 1 + V, kLogKeepMask);
 }
 
 void launch_patch_offset(int V, const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
                          int64_t count, double *part, cudaStream_t s) {
-    const PatchGroup *groups = pa.groups + (V == kOffCoarserSrc ? po.n_groups0 : 0);
-    const int n_groups = V == kOffCoarserSrc ? po.n_groups1 : po.n_groups0;
-    if (count == 0 || n_groups == 0) return;
+    if (count == 0) return;
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(2) * sms));
-#define SG_LAUNCH_OFFSET(VV)                                                                                          \
-    patch_offset_kernel<VV><<<grid, kOffWarps * 32, patch_offset_smem<VV>(), s>>>(                                    \
-        pa.info, pa.levels, groups, pa.pmap, pa.wQ, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,        \
-        po.last_patch, first, count, part, d.queue + 1 + VV, kLogKeepMask)
-    if (V == kOffSame) SG_LAUNCH_OFFSET(0);
-    else if (V == kOffCoarserSrc) SG_LAUNCH_OFFSET(1);
-    else SG_LAUNCH_OFFSET(2);
-#undef SG_LAUNCH_OFFSET
+    switch (V) {
+        case kOffSame: launch_patch_offset_one<kOffSame>(d, pa, po, first, count, part, sms, s); break;
+        case kOffCoarserSrc: launch_patch_offset_one<kOffCoarserSrc>(d, pa, po, first, count, part, sms, s); break;
+        case kOffFinerSrc: launch_patch_offset_one<kOffFinerSrc>(d, pa, po, first, count, part, sms, s); break;
+        case kOffCoarserSrc4: launch_patch_offset_one<kOffCoarserSrc4>(d, pa, po, first, count, part, sms, s); break;
+        default: launch_patch_offset_one<kOffFinerSrc4>(d, pa, po, first, count, part, sms, s); break;
+    }
 }
 
 size_t patch_smem_bytes(int P, int tab_entries) {

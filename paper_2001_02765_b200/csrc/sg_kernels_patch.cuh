@@ -18,16 +18,21 @@ struct PatchLevel {                   // the leaf patches of one level (contiguo
 };
 
 // Pair classes of patch_offset_kernel<V>: source patches of the target's own level (V = 0), of the next coarser
-// level (V = 1) and of the next finer level (V = 2).
-constexpr int kOffSame = 0, kOffCoarserSrc = 1, kOffFinerSrc = 2;
+// level (V = 1), the next finer level (V = 2), two levels coarser (V = 3), two levels finer (V = 4).
+constexpr int kOffSame = 0, kOffCoarserSrc = 1, kOffFinerSrc = 2, kOffCoarserSrc4 = 3, kOffFinerSrc4 = 4;
+constexpr int kOffClasses = 5;
+// Target-patch groups come in three lists: 0 = any 8 patches of a level (classes 0, 2, 4), 1 = 8 patches of one
+// residue class (pi % 2, pj % 2) (class 1), 2 = of one residue class mod 4 (class 3): for a coarser source the source
+// patch of A at offset d is (A + d) / F, which must be integral for the whole group.
+constexpr int offset_group_list(int V) { return V == kOffCoarserSrc ? 1 : V == kOffCoarserSrc4 ? 2 : 0; }
 
-struct PatchGroup {                   // <= 8 target patches of one level (list 1: of one parity class (pi % 2, pj % 2))
+struct PatchGroup {                   // <= 8 target patches of one level (lists 1, 2: of one residue class)
     int32_t level, n;
     int32_t patch[8];                 // patch indices (unused entries: -1)
     int32_t pmin, pmax;               // smallest / largest patch index (target-range test)
     // per pair class: box of patch offsets d that can hit a source patch, in units of the FINER level's patch
-    // size: {dpi_min, ndpi, dpj_min, ndpj}; class 1 steps d by 2 (A + d must be even); ndpi = 0: class absent
-    int32_t box[3][4];
+    // size: {dpi_min, ndpi, dpj_min, ndpj}; classes 1 / 3 step d by 2 / 4 (A + d must be a multiple); ndpi = 0: absent
+    int32_t box[kOffClasses][4];
 };
 
 constexpr int kPatchQStride = 17 * 18;   // doubles per patch in wQ
@@ -57,15 +62,15 @@ struct PatchPlan {
 size_t patch_smem_bytes(int P, int tab_entries);
 cudaError_t configure_patch_kernels(int P, int tab_entries);
 void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s);
-// skip_near: 0 = all patch pairs, 1 = skip pairs of the same level, 2 = skip pairs at most one level apart
+// skip_near: patch pairs fewer than skip_near levels apart are skipped (done by patch_offset_kernel); 0 = none
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
                               int64_t count, double *part, int skip_near, cudaStream_t s);
-// register-blocked kernels with one offset table per CTA (P = 16), patch pairs at most one level apart
+// register-blocked kernels with one offset table per CTA (P = 16), patch pairs at most two levels apart
 struct OffsetPlan {
-    int n_groups0 = 0, n_groups1 = 0; // group list 0 (pair classes 0 and 2) and list 1 (class 1), stored back to back
+    int n_groups[3] = {0, 0, 0};      // sizes of the three group lists, stored back to back
     int n_split = 1;                  // splits of every group's offset list
     int first_patch = 0, last_patch = -1;   // target patches touched by the target range
-    bool variant[3] = {false, false, false};   // pair classes present in this layout
+    bool variant[kOffClasses] = {false, false, false, false, false};   // pair classes present for the target range
 };
 cudaError_t configure_patch_offset();
 // pair class V writes po.n_split slots of [2][count] partial sums at `part` and uses queue counter 1 + V
