@@ -123,12 +123,13 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
  *   SG_MODE_DIRECT   every (target, vertex) pair: 1 sqrt + 2 ln (the north_star kernel; always available; default)
  *   SG_MODE_LATTICE  lattice-offset reuse: per (target patch, source patch) the pair function
  *                    is tabulated once on the patch pair's offset lattice and the pairs reduce to 2 FMA each;
- *                    patch pairs more than one level apart are summed directly.  Needs P = 8 or 16
+ *                    Needs P = 8 or 16
  *                    (SG_ERR_ARG otherwise).  Same sum, same tolerances; the slope path always runs DIRECT.
- *                    Large P = 16 problems (>= 4 target patches per SM) run the register-blocked kernels that
- *                    share one offset table per CTA; smaller ones a lighter one-target-per-thread kernel.
- *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but the register-blocked kernels at any problem size
- *                    (P = 16 only, SG_ERR_ARG otherwise).  For tests and profiling.
+ *                    P = 16 runs the register-blocked kernels that share one offset table per CTA (patch pairs
+ *                    up to two levels apart; farther pairs are summed directly); P = 8 a lighter
+ *                    one-target-per-thread kernel (pairs up to one level apart by table).
+ *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but SG_ERR_ARG unless the register-blocked kernels are
+ *                    available (P = 16).  For tests and profiling.
  */
 #define SG_MODE_DIRECT  0
 #define SG_MODE_LATTICE 1
