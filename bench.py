@@ -89,15 +89,15 @@ def parse_args():
     return ap.parse_args()
 
 
-def measured_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the interaction kernel from the committed ncu
-    capture of this workload (profiles/traffic.csv), or None if no capture exists for it."""
+def measured_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu capture of this
+    workload (profiles/traffic.csv), or None if no capture exists for it."""
     import csv
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(path):
         with open(path) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload:
+                if row["workload"] == workload and kernel.startswith(row["kernel"]):
                     return int(row["dram_bytes_per_launch"])
     return None
 
@@ -316,12 +316,13 @@ def run_ours(args):
             }
 
         direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
-        direct_traffic = measured_traffic(workload_name(args.config)) if world == 1 else None
+        direct_traffic = measured_traffic(workload_name(args.config), direct_name) if world == 1 else None
         if args.slopes:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>", None)
         elif lattice:
-            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps,
-                                   "patch_offset_kernel (+ patch_interaction_kernel on multi-level layouts)", None)
+            lattice_name = "patch_offset_kernel<0> (same-level pairs; <1>..<4> for pairs one and two levels apart)"
+            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, lattice_name,
+                                   measured_traffic(workload_name(args.config), lattice_name) if world == 1 else None)
         else:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, direct_name, direct_traffic)
         line = {
