@@ -5,7 +5,7 @@ import pytest
 
 import oracle
 from test_oracle_pins import F_D2_xy, _agree_3_digits, _norms
-from workloads import (cell_rects, make_config, paper_ilr_layout, sample_targets, d2_sigma, d2_slopes, d22_sigma,
+from workloads import (cell_rects, make_config, paper_ilr_layout, paper_vlr_layout, sample_targets, d2_sigma, d2_slopes, d22_sigma,
                        d22_slopes, nested_layout, kuzmin_sigma)
 from workloads.configs import cell_centres, uniform_layout
 
@@ -156,4 +156,18 @@ def test_paper_table3_ILR_Linf_on_gpu(torch_cuda, golden, L, Nk):
     ax, ay = F_D2_xy(x, y, 0.5)
     R = np.hypot(x, y)
     assert _agree_3_digits(np.abs(Fx - ax).max(), row[2])
+    assert _agree_3_digits(np.abs((Fx * x + Fy * y) / R - (ax * x + ay * y) / R).max(), row[3])
+
+
+@pytest.mark.parametrize("L,Nk", [(2, 128), (3, 128), (2, 256), (3, 256), (2, 512), (3, 512), (2, 1024), (3, 1024)])
+def test_paper_table5_VLR_Linf_on_gpu(torch_cuda, golden, L, Nk):
+    """PAPER.md:274-291 Table 5 L-infinity columns on the paper's VLR quadtrees (P = 1; Table 9's workloads)."""
+    row = [r for r in golden("paper_table5_VLR_Linf.txt") if int(r[0]) == L and int(r[1]) == Nk][0]
+    lay = paper_vlr_layout(Nk, L, "D2")
+    x, y, h = cell_centres(lay)
+    Fx, Fy = gpu_force_linear(torch_cuda, lay, d2_sigma(x, y, 0.5), *d2_slopes(x, y, 0.5))
+    ax, ay = F_D2_xy(x, y, 0.5)
+    R = np.hypot(x, y)
+    if not row[2].endswith("?"):                                   # see the fixture's header for the one misprint
+        assert _agree_3_digits(np.abs(Fx - ax).max(), row[2])
     assert _agree_3_digits(np.abs((Fx * x + Fy * y) / R - (ax * x + ay * y) / R).max(), row[3])

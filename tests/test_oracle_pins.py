@@ -281,6 +281,24 @@ def test_P2_paper_table3_ILR_Linf(golden, L, Nk):
     assert _agree_3_digits(np.abs((Fx * x[q] + Fy * y[q]) / R - (ax * x[q] + ay * y[q]) / R).max(), row[3])
 
 
+@pytest.mark.parametrize("L,Nk", [(2, 128), (3, 128)])
+def test_P2_paper_table5_VLR_Linf(golden, L, Nk):
+    """Second AMR pin, on the paper's other refinement driver (PAPER.md:164 VLR, Table 5): other coincidence
+    patterns than Table 3 (wider refined bands, level-3 zones next to level-1 zones)."""
+    row = [r for r in golden("paper_table5_VLR_Linf.txt") if int(r[0]) == L and int(r[1]) == Nk][0]
+    lay = paper_vlr_layout(Nk, L, "D2")
+    r = cell_rects(lay)
+    x, y, h = cell_centres(lay)
+    sig = d2_sigma(x, y, 0.5)
+    dx, dy = d2_slopes(x, y, 0.5)
+    q = np.nonzero((x > 0) & (y > 0))[0]
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+    ax, ay = F_D2_xy(x[q], y[q], 0.5)
+    R = np.hypot(x[q], y[q])
+    assert _agree_3_digits(np.abs(Fx - ax).max(), row[2])
+    assert _agree_3_digits(np.abs((Fx * x[q] + Fy * y[q]) / R - (ax * x[q] + ay * y[q]) / R).max(), row[3])
+
+
 def test_paper_leaf_counts_tables_8_9(golden):
     for rule, disk, L, Nk, EL in golden("paper_table8_9_leaf_counts.txt"):
         if int(Nk) > 256:
