@@ -171,3 +171,18 @@ def test_paper_table5_VLR_Linf_on_gpu(torch_cuda, golden, L, Nk):
     if not row[2].endswith("?"):                                   # see the fixture's header for the one misprint
         assert _agree_3_digits(np.abs(Fx - ax).max(), row[2])
     assert _agree_3_digits(np.abs((Fx * x + Fy * y) / R - (ax * x + ay * y) / R).max(), row[3])
+
+
+@pytest.mark.parametrize("rule", ["ILR", "VLR"])
+@pytest.mark.parametrize("L,Nk", [(2, 128), (3, 128), (2, 256), (3, 256), (2, 512), (3, 512), (2, 1024), (3, 1024)])
+def test_paper_tables4_6_D22_Linf_on_gpu(torch_cuda, golden, rule, L, Nk):
+    """PAPER.md:235-252 Table 4 (ILR) and :303-320 Table 6 (VLR), double disk, L-infinity of the x and y errors."""
+    row = [r for r in golden("paper_table4_6_D22_Linf.txt") if r[0] == rule and int(r[1]) == L and int(r[2]) == Nk][0]
+    lay = (paper_ilr_layout if rule == "ILR" else paper_vlr_layout)(Nk, L, "D22")
+    x, y, h = cell_centres(lay)
+    Fx, Fy = gpu_force_linear(torch_cuda, lay, d22_sigma(x, y), *d22_slopes(x, y))
+    a1 = F_D2_xy(x, y, 0.4, 0.0, 0.5)
+    a2 = F_D2_xy(x, y, 0.4, 0.0, -0.5)
+    for got, printed in ((np.abs(Fx - a1[0] - a2[0]).max(), row[3]), (np.abs(Fy - a1[1] - a2[1]).max(), row[4])):
+        if not printed.endswith("?"):                              # see the fixture's header
+            assert _agree_3_digits(got, printed), (got, row)

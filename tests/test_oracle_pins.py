@@ -299,6 +299,24 @@ def test_P2_paper_table5_VLR_Linf(golden, L, Nk):
     assert _agree_3_digits(np.abs((Fx * x[q] + Fy * y[q]) / R - (ax * x[q] + ay * y[q]) / R).max(), row[3])
 
 
+@pytest.mark.parametrize("rule,L,Nk", [("ILR", 2, 128), ("ILR", 3, 128), ("VLR", 2, 128)])
+def test_P2_paper_tables4_6_D22_Linf(golden, rule, L, Nk):
+    """AMR pins on the double disk (two refined rings, x and y components differ): Tables 4 (ILR) and 6 (VLR)."""
+    row = [r for r in golden("paper_table4_6_D22_Linf.txt") if r[0] == rule and int(r[1]) == L and int(r[2]) == Nk][0]
+    lay = (paper_ilr_layout if rule == "ILR" else paper_vlr_layout)(Nk, L, "D22")
+    r = cell_rects(lay)
+    x, y, h = cell_centres(lay)
+    sig = d22_sigma(x, y)
+    dx, dy = d22_slopes(x, y)
+    q = np.nonzero((x > 0) & (y > 0))[0]
+    Fx, Fy, _ = oracle.force(r, sig, r["kxc"][q], r["kyc"][q], lay.unit, dx=dx, dy=dy, precision="f64")
+    a1 = F_D2_xy(x[q], y[q], 0.4, 0.0, 0.5)
+    a2 = F_D2_xy(x[q], y[q], 0.4, 0.0, -0.5)
+    for got, printed in ((np.abs(Fx - a1[0] - a2[0]).max(), row[3]), (np.abs(Fy - a1[1] - a2[1]).max(), row[4])):
+        if not printed.endswith("?"):                              # see the fixture's header
+            assert _agree_3_digits(got, printed), (got, row)
+
+
 def test_paper_leaf_counts_tables_8_9(golden):
     for rule, disk, L, Nk, EL in golden("paper_table8_9_leaf_counts.txt"):
         if int(Nk) > 256:
