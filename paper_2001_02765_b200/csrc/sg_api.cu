@@ -222,6 +222,16 @@ int upload_patches(sg_ctx *c) {
                     for (int32_t r = l.p0; r < l.p0 + l.n; ++r)
                         if ((h.patches[size_t(r)].i0 / h.P) % F == cx && (h.patches[size_t(r)].j0 / h.P) % F == cy)
                             members.push_back(r);
+                    // 8 consecutive members should be a compact 4 x 2 block of the class's own patch lattice (pitch F):
+                    // the offset box of a group grows with the group's spread, and every offset costs one table
+                    std::stable_sort(members.begin(), members.end(), [&](int32_t a, int32_t b) {
+                        const sg_patch &pa_ = h.patches[size_t(a)], &pb_ = h.patches[size_t(b)];
+                        const int ai = pa_.i0 / h.P / F, aj = pa_.j0 / h.P / F, bi = pb_.i0 / h.P / F, bj = pb_.j0 / h.P / F;
+                        if ((aj >> 1) != (bj >> 1)) return (aj >> 1) < (bj >> 1);
+                        if ((ai >> 2) != (bi >> 2)) return (ai >> 2) < (bi >> 2);
+                        if (aj != bj) return aj < bj;
+                        return ai < bi;
+                    });
                     for (size_t m0 = 0; m0 < members.size() && ok; m0 += 8) {
                         PatchGroup gr;
                         std::memset(&gr, 0, sizeof gr);
