@@ -106,7 +106,10 @@ int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx
  * S3-S5, the all-pairs sum.  Fx_dev, Fy_dev: device [N] (or [count] when a
  * target range is set, see below), FP64, written in library cell order.  Asynchronous on
  * cuda_stream.  Deterministic: the same context and sigma give bit-identical results run to run
- * (no floating-point atomics).  SG_ERR_STATE if no density has been set.
+ * (no floating-point atomics).  SG_ERR_STATE if no density has been set.  In SG_MODE_LATTICE on a
+ * multi-level layout the independent pair-class kernels run on side streams owned by the context,
+ * forked from and joined back into cuda_stream by events, so for the caller the call still orders
+ * like one piece of work on cuda_stream (and can be captured in a CUDA graph after one warm-up call).
  */
 int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
 

@@ -33,6 +33,11 @@ struct sg_ctx {
     bool timing = false;
     int64_t timed_calls = 0;
     std::vector<cudaEvent_t> ev0, ev1;
+    // lattice mode: the pair-class kernels of one sg_force run concurrently (fork / join around the caller's stream),
+    // so that the tail of one class overlaps the start of the next
+    std::vector<cudaStream_t> side;
+    cudaEvent_t fork_ev = nullptr;
+    std::vector<cudaEvent_t> join_ev;
 };
 
 constexpr int kTimingRing = 64;
@@ -390,6 +395,9 @@ void sg_destroy(sg_ctx *c) {
         for (void *p : c->allocs) cudaFree(p);
         for (cudaEvent_t e : c->ev0) cudaEventDestroy(e);
         for (cudaEvent_t e : c->ev1) cudaEventDestroy(e);
+        for (cudaStream_t st : c->side) cudaStreamDestroy(st);
+        for (cudaEvent_t e : c->join_ev) cudaEventDestroy(e);
+        if (c->fork_ev) cudaEventDestroy(c->fork_ev);
     }
     delete c;
 }
@@ -495,15 +503,41 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
     else if (by_patch) {
-        double *part = c->dev.part;        // every launch writes its own n_split slots of [2][count] partial sums
+        // every launch writes its own n_split slots of [2][count] partial sums and has its own work queue, so the
+        // launches are independent: the first runs on the caller's stream, the others on side streams that wait for
+        // an event recorded on the caller's stream and are joined back into it (capturable in a CUDA graph)
+        double *part = c->dev.part;
+        int n_launch = 0;
+        auto on_stream = [&](int idx) -> cudaStream_t {
+            if (idx == 0) return s;
+            cudaStream_t st = c->side[size_t(idx - 1)];
+            cudaStreamWaitEvent(st, c->fork_ev, 0);
+            return st;
+        };
+        const int n_total = (blocked ? offset_classes(po) : 0) + ((!blocked || far) ? 1 : 0);
+        if (n_total > 1) {
+            while (int(c->side.size()) < n_total - 1) {
+                cudaStream_t st; cudaEvent_t ev;
+                SG_CUDA(c, cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+                c->side.push_back(st);
+                SG_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+                c->join_ev.push_back(ev);
+            }
+            if (!c->fork_ev) SG_CUDA(c, cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
+            SG_CUDA(c, cudaEventRecord(c->fork_ev, s));
+        }
         if (blocked)
             for (int v = 0; v < kOffClasses; ++v)
                 if (po.variant[v]) {
-                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, s);
+                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, on_stream(n_launch++));
                     part += int64_t(po.n_split) * 2 * c->count;
                 }
         if (!blocked || far)
-            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 3 : 0, s);
+            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 3 : 0, on_stream(n_launch++));
+        for (int i = 1; i < n_launch; ++i) {
+            SG_CUDA(c, cudaEventRecord(c->join_ev[size_t(i - 1)], c->side[size_t(i - 1)]));
+            SG_CUDA(c, cudaStreamWaitEvent(s, c->join_ev[size_t(i - 1)], 0));
+        }
     }
     else launch_interaction(c->dev, p, s);
     if (c->timing) {
