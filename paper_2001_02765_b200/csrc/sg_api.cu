@@ -329,6 +329,7 @@ int upload_layout(sg_ctx *c) {
     if ((rc = upload(c, &d.tX, h.tX)) || (rc = upload(c, &d.tY, h.tY))) return rc;
     if ((rc = dev_alloc(c, &d.vtile, int64_t(d.n_tiles) * kTileDoubles))) return rc;
     if ((rc = dev_alloc(c, &d.w, h.Nv))) return rc;
+    if ((rc = dev_alloc(c, &d.wcum, 2 * h.Nv))) return rc;
     if ((rc = dev_alloc(c, &d.TBx, int64_t(d.ntY) * d.nX))) return rc;
     if ((rc = dev_alloc(c, &d.TBy, int64_t(d.ntX) * d.nY))) return rc;
 
@@ -577,8 +578,9 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
 
 int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     if (!c) return SG_ERR_ARG;
-    // vertex weights, column table, row table (+ per-patch weights when the lattice-offset path exists)
-    if (set_density_launches) *set_density_launches = 3 + ((c->patch.enabled && !c->linear) ? 1 : 0);
+    // vertex weights, running sums and look-ups per direction (+ per-patch weights when the lattice-offset path exists);
+    // with slopes: weights, column tables, row tables
+    if (set_density_launches) *set_density_launches = c->linear ? 3 : 5 + (c->patch.enabled ? 1 : 0);
     if (force_launches) {                                         // interaction kernel(s) + finalise
         int n = 1;
         if (c->use_patch && !c->linear && c->count > 0) {

@@ -102,35 +102,50 @@ void launch_fill_static_tiles(const DevLayout &d, cudaStream_t s) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// S2b: cumulative line weights.  One thread per vertex column X (row Y): a merge of the column's
-// vertices (sorted by y) with the sorted distinct target ordinates:
+// S2b: cumulative line weights.
 //   TBx[iy][c] = sum of w over the vertices of column c with y_v <  tY[iy]   (strictly below)
 //   TBy[ix][r] = sum of w over the vertices of row    r with x_v <  tX[ix]   (strictly left)
+// Two steps per direction: a running sum along every line (one thread per line, vertices in line order, so the
+// rounding is that of a plain left-to-right sum), then one thread per (target coordinate, line) finds by bisection
+// how many vertices of the line lie strictly before the coordinate and picks the running sum there.
 // ------------------------------------------------------------------------------------------------
-__global__ void line_tables_kernel(const int32_t *__restrict__ start, const int32_t *__restrict__ perm,
-                                   const int32_t *__restrict__ vcoord, const double *__restrict__ w,
-                                   const int32_t *__restrict__ tcoord, int n_lines, int n_t,
-                                   double *__restrict__ TB) {
+__global__ void line_prefix_kernel(const int32_t *__restrict__ start, const int32_t *__restrict__ perm,
+                                   const double *__restrict__ w, int n_lines, double *__restrict__ wcum) {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_lines) return;
-    int p = start[c];
     const int e = start[c + 1];
     double acc = 0.0;
-    for (int i = 0; i < n_t; ++i) {
-        const int t = tcoord[i];
-        while (p < e) {
-            const int v = perm ? perm[p] : p;
-            if (vcoord[v] >= t) break;
-            acc += w[v];
-            ++p;
-        }
-        TB[int64_t(i) * n_lines + c] = acc;
+    for (int p = start[c]; p < e; ++p) {
+        acc += w[perm ? perm[p] : p];
+        wcum[p] = acc;
     }
 }
 
+__global__ void line_lookup_kernel(const int32_t *__restrict__ start, const int32_t *__restrict__ perm,
+                                   const int32_t *__restrict__ vcoord, const double *__restrict__ wcum,
+                                   const int32_t *__restrict__ tcoord, int n_lines, int n_t, double *__restrict__ TB) {
+    const int64_t idx = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (idx >= int64_t(n_lines) * n_t) return;
+    const int c = int(idx % n_lines), i = int(idx / n_lines);
+    const int t = tcoord[i], s0 = start[c];
+    int lo = s0, hi = start[c + 1];                       // first position in [lo, hi) whose coordinate is >= t
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (vcoord[perm ? perm[mid] : mid] < t) lo = mid + 1; else hi = mid;
+    }
+    TB[idx] = lo > s0 ? wcum[lo - 1] : 0.0;
+}
+
 void launch_line_tables(const DevLayout &d, cudaStream_t s) {
-    line_tables_kernel<<<(d.nX + 127) / 128, 128, 0, s>>>(d.colstart, nullptr, d.vky, d.w, d.tY, d.nX, d.ntY, d.TBx);
-    line_tables_kernel<<<(d.nY + 127) / 128, 128, 0, s>>>(d.rowstart, d.rowperm, d.vkx, d.w, d.tX, d.nY, d.ntX, d.TBy);
+    line_prefix_kernel<<<(d.nX + 63) / 64, 64, 0, s>>>(d.colstart, nullptr, d.w, d.nX, d.wcum);
+    line_prefix_kernel<<<(d.nY + 63) / 64, 64, 0, s>>>(d.rowstart, d.rowperm, d.w, d.nY, d.wcum + d.Nv);
+    const int64_t nx = int64_t(d.nX) * d.ntY, ny = int64_t(d.nY) * d.ntX;
+    if (nx > 0)
+        line_lookup_kernel<<<unsigned((nx + 255) / 256), 256, 0, s>>>(d.colstart, nullptr, d.vky, d.wcum, d.tY, d.nX,
+                                                                     d.ntY, d.TBx);
+    if (ny > 0)
+        line_lookup_kernel<<<unsigned((ny + 255) / 256), 256, 0, s>>>(d.rowstart, d.rowperm, d.vkx, d.wcum + d.Nv, d.tX,
+                                                                     d.nY, d.ntX, d.TBy);
 }
 
 // ------------------------------------------------------------------------------------------------

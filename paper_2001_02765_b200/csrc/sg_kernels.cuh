@@ -34,6 +34,7 @@ struct DevLayout {
     int32_t *slot_vertex = nullptr;   // [n_slots] vertex index or -1
     double *vtile = nullptr;          // [n_tiles * kTileDoubles]
     double *w = nullptr;              // [Nv]
+    double *wcum = nullptr;           // [2 Nv] running sums of w along the columns, then along the rows (S2b scratch)
     int32_t *colX = nullptr, *colstart = nullptr;           // [nX], [nX+1]
     int32_t *rowY = nullptr, *rowstart = nullptr, *rowperm = nullptr;   // [nY], [nY+1], [Nv]
     int32_t *tX = nullptr, *tY = nullptr;                   // [ntX], [ntY]

@@ -116,9 +116,9 @@ def test_host_only_context_never_computes():
         assert lib.sg_set_density(d._ctx, dummy, None) == binding.SG_ERR_CUDA
         assert lib.sg_force(d._ctx, dummy, dummy, None) == binding.SG_ERR_CUDA
         assert b"no CPU fallback" in lib.sg_last_error(d._ctx)
-        assert d.launch_counts() == (3, 2)
+        assert d.launch_counts() == (5, 2)
         d.set_target_range(5, 0)
-        assert d.launch_counts() == (3, 0)
+        assert d.launch_counts() == (5, 0)
         with pytest.raises(SgError):
             d.set_target_range(250, 10)
 
