@@ -102,6 +102,39 @@ def measured_traffic(workload: str, kernel: str):
     return None
 
 
+def amr_side_measurement(torch, device, flush):
+    """BASELINE.json config 4 (three-level AMR, 448,768 leaves) through the same calls, lattice mode: 3 steps of
+    sg_set_density + sg_force between CUDA events after 2 warm-up steps, L2 flushed between steps.  Reported next to
+    the headline (uniform) workload because AMR layouts are what the method is for."""
+    from paper_2001_02765_b200 import SgDisk
+    from workloads import make_config
+    lay4, sigma4 = make_config(4)
+    with SgDisk.from_layout(lay4, device=device) as d4:
+        d4.set_interaction_mode("lattice")
+        s4 = torch.as_tensor(sigma4).to(torch.device("cuda", device))
+        Fx = torch.empty(lay4.n_cells, dtype=torch.float64, device=s4.device)
+        Fy = torch.empty_like(Fx)
+
+        def step():
+            flush.zero_()
+            d4.set_density(s4)
+            d4.force(Fx, Fy)
+        for _ in range(2):
+            step()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(3):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 3
+        sd, fl = d4.launch_counts()
+    return {"workload": workload_name(4), "n_cells": lay4.n_cells, "value": float(lay4.n_cells) ** 2 / (ms * 1e-3),
+            "unit": UNIT, "ms_per_step": ms, "steps": 3, "warmup": 2, "gpu_launches_per_step": sd + fl,
+            "interaction_mode": "lattice-offset reuse (SG_MODE_LATTICE): pair classes up to two levels apart"}
+
+
 def workload_name(cfg: int) -> str:
     from workloads import CONFIG_NAMES
     return CONFIG_NAMES[cfg]
@@ -348,6 +381,8 @@ def run_ours(args):
                         "(the north_star interaction kernel); 2 timed steps after 1 warm-up",
                 "value": pairs * 2 / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / 2,
                 "roofline": roofline_of(d_model, d_k, d_total / 2, direct_name, direct_traffic)}
+        if world == 1 and args.config == 5 and not args.slopes and lattice:
+            line["amr_workload"] = amr_side_measurement(torch, local, flush)
         if not args.no_cpu_baseline and world == 1:
             rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds)
             line["cpu_baseline"] = {
