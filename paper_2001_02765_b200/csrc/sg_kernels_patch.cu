@@ -215,7 +215,6 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     using C = OffCls<V>;
     constexpr int P = 16, F = C::F, M = C::M, MMIN = C::MMIN, TROW = C::TROW, TBUF = C::TBUF;
     constexpr int STEP = C::coarser ? F : 1;                              // offsets keep A + d a multiple of F
-    constexpr int EVALS = (M * M + kOffWarps * 32 - 1) / (kOffWarps * 32);
     // per thread and source row: coarser source: NCLS column classes of MT targets each, NT table steps;
     // otherwise 8 consecutive targets, NT table entries
     constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
@@ -276,18 +275,26 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         };
         // T[row][col] = pair function at u = B.X0 - x_centre(A, k = 0) + (col - MMIN) g, likewise v; for a finer
         // source the rows are stored by row class (row % RA): the 16 lanes of a half-warp read consecutive stored rows
-        auto build = [&](int n, double2 *T) {
+        // Consecutive offsets of one box row shift the table by SHIFT columns: with `prev` (the table of offset n-1,
+        // complete and read-only while table n is built) only the last SHIFT columns are evaluated, the others copied.
+        auto build = [&](int n, double2 *T, const double2 *prev) {
+            constexpr int SHIFT = STEP * P;                               // columns (units of g) between offsets d, d + STEP
             const double u00 = double((dpi_min + STEP * (n % ndpi)) * P) * g - 0.5 * double(lev.cw);
             const double v00 = double((dpj_min + STEP * (n / ndpi)) * P) * g - 0.5 * double(lev.cw);
-#pragma unroll 4
-            for (int q = 0; q < EVALS; ++q) {
-                const int e = tid + q * (kOffWarps * 32), mm = e % M, nn = e / M;
-                if (M * M % (kOffWarps * 32) == 0 || e < M * M) {
-                    const int pos = nn / C::RA + (nn % C::RA) * C::RPC;
-                    T[pos * TROW + mm] = pair_terms_g(fma(double(mm - MMIN), g, u00), fma(double(nn - MMIN), g, v00),
-                                                      lntab_g, tab_idx0, keep);
-                }
+            const bool reuse = SHIFT < M && prev != nullptr && n % ndpi != 0;
+            const int m0 = reuse ? M - SHIFT : 0, ncol = M - m0;          // columns [m0, M) are evaluated
+#pragma unroll 2
+            for (int e = tid; e < M * ncol; e += kOffWarps * 32) {
+                const int mm = m0 + e % ncol, nn = e / ncol;
+                const int pos = nn / C::RA + (nn % C::RA) * C::RPC;
+                T[pos * TROW + mm] = pair_terms_g(fma(double(mm - MMIN), g, u00), fma(double(nn - MMIN), g, v00),
+                                                  lntab_g, tab_idx0, keep);
             }
+            if (reuse)
+                for (int e = tid; e < C::ROWS * m0; e += kOffWarps * 32) {
+                    const int mm = e % m0, pos = e / m0;
+                    T[pos * TROW + mm] = prev[pos * TROW + mm + SHIFT];
+                }
         };
         auto consume = [&](int b, const double2 *T) {
             // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
@@ -337,12 +344,12 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         bool any_cur = false, any_next = false;
         int b_cur = lookup(n0, any_cur), b_next = -1;
         if (C::DB) {
-            if (any_cur) build(n0, sT);
+            if (any_cur) build(n0, sT, nullptr);
             __syncthreads();
             for (int n = n0; n < n1; ++n) {
                 b_next = lookup(n + 1, any_next);
                 if (!any_cur && !any_next) continue;             // nothing built, nothing consumed: no barrier needed
-                if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * TBUF);
+                if (any_next) build(n + 1, sT + ((n + 1 - n0) & 1) * TBUF, any_cur ? sT + ((n - n0) & 1) * TBUF : nullptr);
                 if (my_patch >= 0 && b_cur >= 0) consume(b_cur, sT + ((n - n0) & 1) * TBUF);
                 __syncthreads();
                 b_cur = b_next; any_cur = any_next;
@@ -350,7 +357,7 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         } else {                                                 // one table buffer: build, barrier, consume, barrier
             for (int n = n0; n < n1; ++n) {
                 if (any_cur) {
-                    build(n, sT);
+                    build(n, sT, nullptr);
                     __syncthreads();
                     if (my_patch >= 0 && b_cur >= 0) consume(b_cur, sT);
                     __syncthreads();
