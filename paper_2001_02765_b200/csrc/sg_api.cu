@@ -245,7 +245,10 @@ int upload_patches(sg_ctx *c) {
                         int64_t gimin = INT32_MAX, gimax = INT32_MIN, gjmin = INT32_MAX, gjmax = INT32_MIN;
                         gr.pmin = INT32_MAX; gr.pmax = INT32_MIN;
                         for (int w = 0; w < 8; ++w) {
-                            gr.patch[w] = w < gr.n ? members[m0 + size_t(w)] : -1;
+                            // warp w runs on SM sub-partition w % 4: rotate the block's second row by one so that the two
+                            // patches of a block column (idle together at the edge of the level) sit on different ones
+                            const int src = (gr.n == 8 && w >= 4) ? 4 + ((w - 4 + 3) & 3) : w;
+                            gr.patch[w] = w < gr.n ? members[m0 + size_t(src)] : -1;
                             if (w >= gr.n) continue;
                             const sg_patch &q = h.patches[size_t(gr.patch[w])];
                             gimin = std::min<int64_t>(gimin, q.i0 / h.P); gimax = std::max<int64_t>(gimax, q.i0 / h.P);
