@@ -139,6 +139,19 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 #define SG_MODE_LATTICE_BLOCKED 2
 int sg_set_interaction_mode(sg_ctx *ctx, int mode);
 
+/*
+ * Diagnostic of the SG_MODE_LATTICE launch plan (P = 16), computed on the host (works on a context created with
+ * device < 0): replays the walk of the offset-table kernels over every target group and patch offset and counts
+ * the (target patch, source patch) pairs it reaches.  out[12]:
+ *   out[0..4]  pairs reached per pair class: same level, source one level coarser, one finer, two coarser, two finer
+ *   out[5]     pairs reached more than once (must be 0)      out[6]  pairs of the wrong level distance (must be 0)
+ *   out[7..9]  target groups in the three group lists         out[10] offsets visited (= offset tables at most)
+ *   out[11]    1 if the plan exists (P = 16, patch maps fit), else 0 and everything else is 0
+ * Every patch pair at most two levels apart must be reached exactly once; pairs farther apart are summed directly.
+ * Only for layouts of at most 65,536 patches (larger: counts stay 0).
+ */
+int sg_lattice_plan_check(const sg_ctx *ctx, int64_t *out);
+
 /* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
 int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
 

@@ -20,7 +20,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 # every symbol include/sg_disk.h declares (tests check the header and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
-    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
+    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
@@ -77,6 +77,8 @@ def load_library():
     lib.sg_set_target_range.argtypes = [vp, c_i64, c_i64]
     lib.sg_set_interaction_mode.restype = c_int
     lib.sg_set_interaction_mode.argtypes = [vp, c_int]
+    lib.sg_lattice_plan_check.restype = c_int
+    lib.sg_lattice_plan_check.argtypes = [vp, ctypes.POINTER(c_i64)]
     lib.sg_launch_counts.restype = c_int
     lib.sg_launch_counts.argtypes = [vp, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
     lib.sg_set_kernel_timing.restype = c_int
@@ -204,6 +206,14 @@ class SgDisk:
         """'direct' (every pair: sqrt + 2 ln), 'lattice' (per-patch-pair offset tables; P = 8 or 16) or
         'lattice_blocked' (the register-blocked offset-table kernels at any size; P = 16)."""
         self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1, "lattice_blocked": 2}[mode]))
+
+    def lattice_plan_check(self):
+        """Host-side replay of the lattice-mode launch plan (see sg_lattice_plan_check)."""
+        out = (ctypes.c_int64 * 12)()
+        self._check(self._lib.sg_lattice_plan_check(self._ctx, out))
+        v = list(out)
+        return {"pairs_per_class": v[0:5], "duplicates": v[5], "wrong_level": v[6], "groups": v[7:10],
+                "offsets": v[10], "available": bool(v[11])}
 
     def force(self, Fx=None, Fy=None):
         """Fx, Fy (CUDA float64 [count]) at the leaf centres of the current target range."""

@@ -22,7 +22,11 @@ struct sg_ctx {
     bool linear = false;         // last density call carried slopes (sg_set_density_linear)
     LinArrays lin;
     PatchArrays patch;           // lattice-offset reuse path (P = 8 or 16)
-    std::vector<PatchGroup> patch_groups;   // host copy of patch.groups (launch planning): list 0 then list 1
+    std::vector<PatchInfo> patch_info;      // host side of the lattice path (build_patch_plan)
+    std::vector<PatchLevel> patch_levels;
+    std::vector<int32_t> patch_pmap;
+    bool patch_plan_ok = false;             // P == 16 and the per-level patch maps fit
+    std::vector<PatchGroup> patch_groups;   // the three group lists back to back (offset_group_list)
     int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
     bool use_patch = false;      // sg_set_interaction_mode
     int64_t first = 0, count = 0;
@@ -165,27 +169,24 @@ int offset_classes(const OffsetPlan &po) {
 // cfg 1: 25 vs 37 us, cfg 3: 2.6 vs 4.0 ms); P = 8: generic kernel
 bool use_blocked(const sg_ctx *c, const PatchPlan &) { return c->patch.blocked; }
 
-int upload_patches(sg_ctx *c) {
+// Host-side plan of the offset-table kernels (P = 16): per-patch lattice info, per-level dense patch maps, target
+// groups with their offset boxes per pair class.  No CUDA: also built for host-only contexts (sg_lattice_plan_check).
+bool build_patch_plan(sg_ctx *c) {
     const HostLayout &h = c->host;
-    PatchArrays &pa = c->patch;
-    if (h.P != 8 && h.P != 16) return SG_OK;                               // direct kernel only
-    pa.P = h.P;
-    pa.n_patches = int(h.patches.size());
-    pa.wstride = ((h.P + 1) * (h.P + 1) + 1) & ~1;
-    std::vector<PatchInfo> info(h.patches.size());
+    std::vector<PatchInfo> &info = c->patch_info;
+    info.resize(h.patches.size());
     for (size_t p = 0; p < info.size(); ++p) {
         const int32_t cw = int32_t(2) << (h.n_levels - 1 - h.patches[p].level);
         info[p] = PatchInfo{h.patches[p].i0 * cw, h.patches[p].j0 * cw, cw, h.patches[p].level};
     }
-    int rc;
-    if ((rc = upload(c, &pa.info, info))) return rc;
-    if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
-    SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
-    if (pa.P == 16) {
+    if (h.P != 16) return false;
+    {
         // per level: dense map patch position -> patch index; groups of <= 8 consecutive patches with the box of
         // patch offsets that can reach a source patch of the same level (patch_offset_kernel)
-        std::vector<PatchLevel> lev(size_t(h.n_levels), PatchLevel{0, 0, 0, 0, 0, 0, 0, 0});
-        std::vector<int32_t> pmap;
+        std::vector<PatchLevel> &lev = c->patch_levels;
+        lev.assign(size_t(h.n_levels), PatchLevel{0, 0, 0, 0, 0, 0, 0, 0});
+        std::vector<int32_t> &pmap = c->patch_pmap;
+        pmap.clear();
         std::vector<PatchGroup> &groups = c->patch_groups;
         groups.clear();
         int64_t map_total = 0;
@@ -290,6 +291,26 @@ int upload_patches(sg_ctx *c) {
             c->patch_n_groups[list] = int(glist[list].size());
             groups.insert(groups.end(), glist[list].begin(), glist[list].end());
         }
+        return ok;
+    }
+}
+
+int upload_patches(sg_ctx *c) {
+    const HostLayout &h = c->host;
+    PatchArrays &pa = c->patch;
+    if (h.P != 8 && h.P != 16) return SG_OK;                               // direct kernel only
+    pa.P = h.P;
+    pa.n_patches = int(h.patches.size());
+    pa.wstride = ((h.P + 1) * (h.P + 1) + 1) & ~1;
+    int rc;
+    if ((rc = upload(c, &pa.info, c->patch_info))) return rc;
+    if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
+    SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
+    if (pa.P == 16) {
+        const bool ok = c->patch_plan_ok;
+        const std::vector<PatchLevel> &lev = c->patch_levels;
+        const std::vector<int32_t> &pmap = c->patch_pmap;
+        const std::vector<PatchGroup> &groups = c->patch_groups;
         if (ok) {
             if ((rc = upload(c, &pa.levels, lev)) || (rc = upload(c, &pa.groups, groups)) || (rc = upload(c, &pa.pmap, pmap)))
                 return rc;
@@ -371,6 +392,7 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
         c->device = device;
         c->dev.G = G;
         c->first = 0; c->count = c->host.N;
+        c->patch_plan_ok = build_patch_plan(c);
         if (device >= 0) {
             cudaError_t e = cudaSetDevice(device);
             if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -576,6 +598,52 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
         c->err = "target range outside [0, N)"; return SG_ERR_ARG;
     }
     c->first = first; c->count = count;
+    return SG_OK;
+}
+
+int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
+    if (!c || !out) return SG_ERR_ARG;
+    for (int i = 0; i < 12; ++i) out[i] = 0;
+    if (!c->patch_plan_ok) return SG_OK;
+    out[11] = 1;
+    const HostLayout &h = c->host;
+    const int64_t np = int64_t(h.patches.size());
+    if (np * np > (int64_t(1) << 32)) return SG_OK;                       // diagnostic for test-sized layouts
+    std::vector<uint8_t> hits(size_t(np * np), 0);
+    const int F_of[kOffClasses] = {1, 2, 2, 4, 4}, dl_of[kOffClasses] = {0, -1, 1, -2, 2};
+    size_t g0 = 0;
+    for (int list = 0; list < 3; ++list) {
+        out[7 + list] = c->patch_n_groups[list];
+        for (size_t gi = g0; gi < g0 + size_t(c->patch_n_groups[list]); ++gi) {
+            const PatchGroup &g = c->patch_groups[gi];
+            for (int v = 0; v < kOffClasses; ++v) {
+                if (offset_group_list(v) != list) continue;
+                const int ndpi = g.box[v][1], ndpj = g.box[v][3];
+                if (ndpi * ndpj == 0) continue;
+                const int F = F_of[v], step = dl_of[v] < 0 ? F : 1;
+                const PatchLevel &slev = c->patch_levels[size_t(g.level + dl_of[v])];
+                out[10] += int64_t(ndpi) * ndpj;
+                for (int n = 0; n < ndpi * ndpj; ++n)                          // the walk of patch_offset_kernel<v>
+                    for (int w = 0; w < g.n; ++w) {
+                        const int api = h.patches[size_t(g.patch[w])].i0 / h.P, apj = h.patches[size_t(g.patch[w])].j0 / h.P;
+                        const int dx = g.box[v][0] + step * (n % ndpi), dy = g.box[v][2] + step * (n / ndpi);
+                        int bi, bj;
+                        if (dl_of[v] < 0) {
+                            if ((api + dx) % F != 0 || (apj + dy) % F != 0) { ++out[6]; continue; }
+                            bi = (api + dx) / F; bj = (apj + dy) / F;
+                        } else { bi = F * api + dx; bj = F * apj + dy; }
+                        bi -= slev.pimin; bj -= slev.pjmin;
+                        if (bi < 0 || bi >= slev.npx || bj < 0 || bj >= slev.npy) continue;
+                        const int b = c->patch_pmap[size_t(slev.map_off) + size_t(bj) * slev.npx + bi];
+                        if (b < 0) continue;
+                        if (h.patches[size_t(b)].level - g.level != dl_of[v]) ++out[6];
+                        if (hits[size_t(g.patch[w]) * np + b]++) ++out[5];
+                        ++out[v];
+                    }
+            }
+        }
+        g0 += size_t(c->patch_n_groups[list]);
+    }
     return SG_OK;
 }
 

@@ -10,7 +10,8 @@ import pytest
 
 import paper_2001_02765_b200 as sgd
 from paper_2001_02765_b200 import SgDisk, SgError, binding
-from workloads import Layout, make_config, cell_rects, expected_counts, paper_ilr_layout
+from workloads import (Layout, make_config, cell_rects, expected_counts, paper_ilr_layout, nested_layout,
+                       random_refined_layout)
 from workloads.configs import cell_centres, _sorted_patches, uniform_layout
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -131,3 +132,40 @@ def test_shard_range_partitions_targets():
             for (f0, c0), (f1, _) in zip(pieces, pieces[1:]):
                 assert f0 + c0 == f1
             assert max(c for _, c in pieces) - min(c for _, c in pieces) <= 1
+
+
+def _near_pair_counts(lay):
+    """(target patch, source patch) pairs by level distance: same, source 1 coarser, 1 finer, 2 coarser, 2 finer."""
+    cnt = np.bincount(lay.patches[:, 0], minlength=lay.n_levels).astype(np.int64)
+    L = lay.n_levels
+    return [int(np.sum(cnt * cnt)),
+            int(sum(cnt[l] * cnt[l - 1] for l in range(1, L))), int(sum(cnt[l] * cnt[l + 1] for l in range(L - 1))),
+            int(sum(cnt[l] * cnt[l - 2] for l in range(2, L))), int(sum(cnt[l] * cnt[l + 2] for l in range(L - 2)))]
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4", "nest5", "rand1", "rand2", "rand3", "gap"])
+def test_lattice_plan_reaches_every_near_patch_pair_exactly_once(name):
+    """Host replay of the walk of the offset-table kernels (groups x offsets x warps, the same index arithmetic as
+    patch_offset_kernel): every patch pair at most two levels apart is reached exactly once, in the right class."""
+    if name.startswith("cfg"):
+        lay = make_config(int(name[3:]))[0]
+    elif name == "nest5":
+        lay = nested_layout(5, 64, 8.0, 16)
+    elif name == "gap":                                            # levels 0 and 2 only: level 1 has no leaf patch
+        lay = Layout(3, np.array([1.0, 0.5, 0.25]), 0.0, 0.0, 16,
+                     _sorted_patches([(0, 16, 0), (0, 0, 16), (0, 16, 16)] +
+                                     [(2, 16 * i, 16 * j) for j in range(4) for i in range(4)]))
+    else:
+        lay = random_refined_layout(int(name[4:]), 7, 16, 4, 0.35)
+    with SgDisk.from_layout(lay, device=-1) as d:
+        r = d.lattice_plan_check()
+    assert r["available"] and r["duplicates"] == 0 and r["wrong_level"] == 0
+    assert r["pairs_per_class"] == _near_pair_counts(lay)
+    n_groups0 = sum((c + 7) // 8 for c in np.bincount(lay.patches[:, 0]))
+    assert r["groups"][0] == n_groups0
+
+
+def test_lattice_plan_absent_for_other_patch_sizes():
+    lay, _ = make_config(2)                                        # P = 8: generic lattice kernel, no offset plan
+    with SgDisk.from_layout(lay, device=-1) as d:
+        assert not d.lattice_plan_check()["available"]
