@@ -10,7 +10,12 @@
 // a correlation with the patch's own signed vertex weights w^B (cells of B only; the weights of all patches at a
 // shared vertex add up to the deduplicated w_v, so the sum over patches is the same sum):
 //     M^x[l][k] += sum_{j,i} w^B[j][i] T[j rb - l ra][i rb - k ra].x          (2 DFMA per pair)
-// Patch pairs more than one level apart (large M) are summed directly, pair by pair, in the same kernel.
+// Two families of kernels:
+//   patch_offset_kernel<V>       P = 16: one table per CTA shared by 8 target patches, 8 targets per thread, patch pairs
+//                                up to two levels apart (five pair classes V);
+//   patch_interaction_kernel<P>  P = 8 (one target per thread, one table per patch pair, pairs up to one level apart)
+//                                and, for both P, the pairs farther apart (M^2 exceeds the pair count: no reuse left),
+//                                which it sums directly, pair by pair.
 // The separable ln|u| part, the coincidence rule and the epilogue are unchanged (finalise_kernel).
 #include <algorithm>
 
@@ -141,24 +146,27 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 }
 
 // ------------------------------------------------------------------------------------------------
-// Patch pairs at most one level apart, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
+// Patch pairs at most two levels apart, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
 //
 // The table of a patch pair depends only on the patch offset d = B - A (in units of the finer level's patch size)
-// and on the pair class V: source level = target level (V = 0), one level coarser (V = 1), one level finer (V = 2).
-// A CTA takes a group of up to 8 target patches A_w of one level (one warp each; all of one parity class
-// (pi % 2, pj % 2), so that for V = 1 the coarse patch at (A_w + d) / 2 exists for all of them or none) and walks over
-// the offsets d of the class's box; for each d warp w looks up its source patch B_w in the source level's dense patch
-// map (absent: the warp skips this offset).  All 256 threads tabulate T(d) together (4-9 pair-function evaluations
-// per thread instead of 32-72 with a table per warp), double-buffered: the table of offset n+1 is built while offset n
-// is consumed, one CTA barrier per offset.  The log table of the pair function is read through L1.
+// and on the pair class V (sg_kernels_patch.cuh): source level = target level (V = 0), F = 2 or 4 times coarser
+// (V = 1, 3), F = 2 or 4 times finer (V = 2, 4).  A CTA takes a group of up to 8 target patches A_w of one level, one
+// warp each (for a coarser source all of one residue class (pi, pj) mod F, so that the source patch (A_w + d) / F is
+// integral for all of them or none) and walks over the offsets d of the class's box; for each d warp w looks up its
+// source patch B_w in the source level's dense patch map (absent: the warp skips this offset).  All 256 threads
+// tabulate T(d) together, double-buffered for F <= 2 (the table of offset n+1 is built while offset n is consumed, one
+// CTA barrier per offset; consecutive offsets of a box row reuse the overlapping columns of the previous table); the
+// 80 x 80 tables of F = 4 are single-buffered, one CTA per SM.  The log table of the pair function is read through L1.
 //
 // Correlation, 8 targets per thread, lane = l + 16 h (l = target row).  With vertex (i, j) of B and target (k, l) of A
-// the table entry is T[j rb - l ra + 15 ra][i rb - k ra + 15 ra]:
-//   V = 0 (ra = rb = 1): thread owns columns k = 8 h + r; entry column t + 8 - 8 h serves vertices i = t + r - 7;
-//   V = 1 (ra = 1, rb = 2): thread owns the columns of one parity, k = 2 r + h; entry column 2 t + 1 - h serves i = t + r - 7;
-//   V = 2 (ra = 2, rb = 1): thread owns k = 8 h + r; entry column t + 16 - 16 h serves i = t + 2 r - 14; table rows are
-//          stored even rows first (row j - 2 l + 30 has the parity of j, so the 16 lanes read consecutive stored rows).
-// One loaded entry serves the 8 targets of a thread (16 DFMA per LDS.128); the vertex weights sit in registers
+// the table entry is T[j rb - l ra + 15 ra][i rb - k ra + 15 ra] (ra, rb = target / source pitch in units of g):
+//   same level (ra = rb = 1): thread owns columns k = 8 h + r; entry column t + 8 - 8 h serves vertices i = t + r - 7;
+//   coarser source (ra = 1, rb = F): thread owns NCLS = F / 2 column classes mod F of MT = 8 / NCLS targets,
+//          k = F m + NCLS h + cc; entry column F t + F (1 - MT) + 15 - NCLS h - cc serves i = t + m - (MT - 1);
+//   finer source (ra = F, rb = 1): thread owns k = 8 h + r; entry column t + 8 F (1 - h) serves i = t + F r - 7 F;
+//          table rows are stored by row class (row j - F l + 15 F has the residue of j mod F, so the 16 lanes of a
+//          half-warp read consecutive stored rows).
+// One loaded entry serves up to 8 targets of a thread (16 DFMA per LDS.128); the vertex weights sit in registers
 // (fully unrolled, compile-time indices; the ragged ends are removed at compile time).  Stored table rows are an odd
 // number of entries apart so that the 8 lanes of an LDS.128 quarter-warp hit 8 different 16-byte bank groups.
 // Every per-patch sum stays in one accumulator chain (split chains cancel badly).
