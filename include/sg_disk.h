@@ -110,6 +110,8 @@ int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx
  * multi-level layout the independent pair-class kernels run on side streams owned by the context,
  * forked from and joined back into cuda_stream by events, so for the caller the call still orders
  * like one piece of work on cuda_stream (and can be captured in a CUDA graph after one warm-up call).
+ * Test aid: with the environment variable SG_POISON_PARTIALS set, the internal partial-sum buffer is filled
+ * with NaN when it is (re)allocated, so that a partial sum no kernel wrote would surface in Fx, Fy.
  */
 int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
 
@@ -142,11 +144,13 @@ int sg_set_interaction_mode(sg_ctx *ctx, int mode);
 /*
  * Diagnostic of the SG_MODE_LATTICE launch plan (P = 16), computed on the host (works on a context created with
  * device < 0): replays the walk of the offset-table kernels over every target group and patch offset and counts
- * the (target patch, source patch) pairs it reaches.  out[12]:
+ * the (target patch, source patch) pairs it reaches.  out[16]:
  *   out[0..4]  pairs reached per pair class: same level, source one level coarser, one finer, two coarser, two finer
  *   out[5]     pairs reached more than once (must be 0)      out[6]  pairs of the wrong level distance (must be 0)
  *   out[7..9]  target groups in the three group lists         out[10] offsets visited (= offset tables at most)
  *   out[11]    1 if the plan exists (P = 16, patch maps fit), else 0 and everything else is 0
+ *   out[12]    target patches that are not exactly once in a group list whose pair classes are launched (must be 0:
+ *              every launched class writes the partial sums of every target)      out[13..15] reserved, 0
  * Every patch pair at most two levels apart must be reached exactly once; pairs farther apart are summed directly.
  * Only for layouts of at most 65,536 patches (larger: counts stay 0).
  */

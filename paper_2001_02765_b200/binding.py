@@ -209,11 +209,11 @@ class SgDisk:
 
     def lattice_plan_check(self):
         """Host-side replay of the lattice-mode launch plan (see sg_lattice_plan_check)."""
-        out = (ctypes.c_int64 * 12)()
+        out = (ctypes.c_int64 * 16)()
         self._check(self._lib.sg_lattice_plan_check(self._ctx, out))
         v = list(out)
         return {"pairs_per_class": v[0:5], "duplicates": v[5], "wrong_level": v[6], "groups": v[7:10],
-                "offsets": v[10], "available": bool(v[11])}
+                "offsets": v[10], "available": bool(v[11]), "patches_missing_from_launched_lists": v[12]}
 
     def force(self, Fx=None, Fy=None):
         """Fx, Fy (CUDA float64 [count]) at the leaf centres of the current target range."""

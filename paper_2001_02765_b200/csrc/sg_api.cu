@@ -1,6 +1,7 @@
 // sg_api.cu -- the C ABI of include/sg_disk.h: context ownership, uploads, launch planning.
 #include <algorithm>
 #include <climits>
+#include <cstdlib>
 #include <cmath>
 #include <cstring>
 #include <string>
@@ -118,6 +119,9 @@ int ensure_partials(sg_ctx *c, const ForcePlan &p) {
     int rc = dev_alloc(c, &c->dev.part, need);
     if (rc) return rc;
     c->dev.part_capacity = need;
+    // test aid (tests/conftest.py sets it): NaN-fill the partial sums, so that a slot no kernel writes shows up in the
+    // forces instead of passing as a lucky zero of fresh device memory
+    if (std::getenv("SG_POISON_PARTIALS")) SG_CUDA(c, cudaMemset(c->dev.part, 0xFF, size_t(need) * sizeof(double)));
     return SG_OK;
 }
 
@@ -221,7 +225,9 @@ bool build_patch_plan(sg_ctx *c) {
             if (l.n == 0) continue;
             for (int list = 0; list < 3 && ok; ++list) {
                 const int F = 1 << list;                                // residue classes mod F
-                if (list > 0 && !level_ok(L - list)) continue;
+                // a level without a source level `list` levels up still gets its groups in that list (with an empty
+                // box): every launched class must write its partial-sum slots for EVERY target patch
+                const bool has_src = list == 0 || level_ok(L - list);
                 for (int cls = 0; cls < F * F && ok; ++cls) {
                     const int cx = cls % F, cy = cls / F;
                     std::vector<int32_t> members;
@@ -276,7 +282,7 @@ bool build_patch_plan(sg_ctx *c) {
                                 set_box(dl == 1 ? kOffFinerSrc : kOffFinerSrc4, f0.pimin - Ff * gimax, hi_i(f0) - Ff * gimin,
                                         f0.pjmin - Ff * gjmax, hi_j(f0) - Ff * gjmin, 1);
                             }
-                        } else {                                         // source patch (A + d) / F inside the coarser level's box
+                        } else if (has_src) {                            // source patch (A + d) / F inside the coarser level's box
                             const PatchLevel &c0 = lev[size_t(L - list)];
                             set_box(list == 1 ? kOffCoarserSrc : kOffCoarserSrc4, F * int64_t(c0.pimin) - gimax, F * hi_i(c0) - gimin,
                                     F * int64_t(c0.pjmin) - gjmax, F * hi_j(c0) - gjmin, F);
@@ -603,7 +609,7 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
 
 int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
     if (!c || !out) return SG_ERR_ARG;
-    for (int i = 0; i < 12; ++i) out[i] = 0;
+    for (int i = 0; i < 16; ++i) out[i] = 0;
     if (!c->patch_plan_ok) return SG_OK;
     out[11] = 1;
     const HostLayout &h = c->host;
@@ -614,6 +620,17 @@ int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
     size_t g0 = 0;
     for (int list = 0; list < 3; ++list) {
         out[7 + list] = c->patch_n_groups[list];
+        // a list whose classes are launched must hold every patch exactly once (each launch writes the partial sums
+        // of all targets, zeros included)
+        bool launched = false;
+        std::vector<int> seen(size_t(np), 0);
+        for (size_t gi = g0; gi < g0 + size_t(c->patch_n_groups[list]); ++gi) {
+            const PatchGroup &g = c->patch_groups[gi];
+            for (int v = 0; v < kOffClasses; ++v) launched = launched || (offset_group_list(v) == list && g.box[v][1] > 0);
+            for (int w = 0; w < g.n; ++w) ++seen[size_t(g.patch[w])];
+        }
+        if (launched)
+            for (int64_t q = 0; q < np; ++q) out[12] += seen[size_t(q)] != 1;
         for (size_t gi = g0; gi < g0 + size_t(c->patch_n_groups[list]); ++gi) {
             const PatchGroup &g = c->patch_groups[gi];
             for (int v = 0; v < kOffClasses; ++v) {

@@ -9,6 +9,10 @@ if ROOT not in sys.path:
 
 GOLDEN = os.path.join(ROOT, "tests", "golden")
 
+# the library NaN-fills its partial-sum buffer at allocation when this is set: a slot that no kernel writes then shows
+# up as NaN in Fx, Fy instead of passing as a lucky zero of fresh device memory (see ensure_partials in sg_api.cu)
+os.environ.setdefault("SG_POISON_PARTIALS", "1")
+
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")

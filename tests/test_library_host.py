@@ -160,6 +160,7 @@ def test_lattice_plan_reaches_every_near_patch_pair_exactly_once(name):
     with SgDisk.from_layout(lay, device=-1) as d:
         r = d.lattice_plan_check()
     assert r["available"] and r["duplicates"] == 0 and r["wrong_level"] == 0
+    assert r["patches_missing_from_launched_lists"] == 0
     assert r["pairs_per_class"] == _near_pair_counts(lay)
     n_groups0 = sum((c + 7) // 8 for c in np.bincount(lay.patches[:, 0]))
     assert r["groups"][0] == n_groups0
