@@ -7,7 +7,7 @@ import pytest
 
 import oracle
 from workloads import (Layout, make_config, cell_rects, sample_targets, paper_ilr_layout, nested_layout, kuzmin_sigma,
-                       random_refined_layout)
+                       random_refined_layout, make_config4_variant)
 from workloads.configs import cell_centres
 
 pytestmark = pytest.mark.gpu
@@ -144,6 +144,33 @@ def test_blocked_kernels_single_level_and_single_patch(torch_cuda):
     sigma1 = np.random.default_rng(5).uniform(0.5, 1.5, one.n_cells)
     gx, gy = gpu_force(torch_cuda, one, sigma1, "lattice_blocked")
     check(gx, gy, *oracle_force(one, sigma1, np.arange(one.n_cells)))
+
+
+def test_four_level_gradient_refined_layout_at_scale(torch_cuda):
+    """Config 4 with level cap 3 (1,342,720 leaves, four levels: all five pair classes with split offset lists, plus
+    direct far pairs), both modes on ONE context (the partial-sum buffer is re-used and re-sized between them):
+    lattice vs direct everywhere, lattice vs the oracle on a stratified sample."""
+    from paper_2001_02765_b200 import SgDisk
+    lay, sigma = make_config4_variant(3)
+    assert lay.n_cells == 1342720 and lay.n_levels == 4
+    res = {}
+    with SgDisk.from_layout(lay, device=0) as d:
+        d.set_density(torch_cuda.as_tensor(sigma).cuda())
+        for mode in ("direct", "lattice", "direct", "lattice"):
+            d.set_interaction_mode(mode)
+            Fx, Fy = d.force()
+            torch_cuda.cuda.synchronize()
+            got = (Fx.cpu().numpy(), Fy.cpu().numpy())
+            if mode in res:                                        # bit-identical when a mode comes round again
+                assert np.array_equal(res[mode][0], got[0]) and np.array_equal(res[mode][1], got[1])
+            res[mode] = got
+    (dx, dy), (gx, gy) = res["direct"], res["lattice"]
+    s = max(np.abs(dx).max(), np.abs(dy).max())
+    assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
+    assert max(np.abs(gx - dx).max(), np.abs(gy - dy).max()) <= 1e-12 * s
+    idx = sample_targets(lay, 160, 2043)
+    ox, oy = oracle_force(lay, sigma, idx)
+    check(gx[idx], gy[idx], ox, oy)
 
 
 def test_unsupported_patch_size_is_refused(torch_cuda):

@@ -7,4 +7,5 @@ may import this.
 """
 from .configs import (Layout, CONFIG_NAMES, make_config, cell_rects, expected_counts,
                       sample_targets, paper_ilr_layout, paper_vlr_layout, d2_sigma,
-                      d2_slopes, d22_sigma, d22_slopes, nested_layout, kuzmin_sigma, random_refined_layout)
+                      d2_slopes, d22_sigma, d22_slopes, nested_layout, kuzmin_sigma, random_refined_layout,
+                      make_config4_variant)

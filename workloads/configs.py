@@ -293,6 +293,14 @@ def make_config(cfg: int):
     raise ValueError(f"unknown config {cfg}")
 
 
+def make_config4_variant(max_level: int):
+    """BASELINE.json config 4 with another level cap (DESIGN.md R14: the frozen config uses cap 2 = 448,768 leaves;
+    cap 3 gives 1,342,720 leaves on four levels, the literal cap 5 gives 12,150,016 on six)."""
+    lay = _gradient_refined_layout(_ppd_sigma, 256, -1.2, -1.2, 2.4 / 256, 16, max_level=max_level)
+    x, y, _ = cell_centres(lay)
+    return lay, _ppd_sigma(x, y)
+
+
 def sample_targets(lay: Layout, n: int, seed: int) -> np.ndarray:
     """n distinct cell indices, stratified by level (equal share per level, remainder to the
     finest), drawn without replacement with default_rng(seed)."""
