@@ -207,26 +207,26 @@ bool build_patch_plan(sg_ctx *c) {
         std::vector<PatchGroup> &groups = c->patch_groups;
         groups.clear();
         int64_t map_total = 0;
-        size_t p = 0;
         bool ok = true;
-        while (p < info.size() && ok) {
-            const int L = h.patches[p].level;
-            size_t q = p;
+        // the patch list may come in any order: collect the patches of every level (PatchLevel.p0 is unused then)
+        std::vector<std::vector<int32_t>> of_level(size_t(h.n_levels));
+        for (size_t p = 0; p < info.size(); ++p) of_level[size_t(h.patches[p].level)].push_back(int32_t(p));
+        for (int L = 0; L < h.n_levels && ok; ++L) {
+            const std::vector<int32_t> &m = of_level[size_t(L)];
+            if (m.empty()) continue;
             int imin = INT32_MAX, imax = INT32_MIN, jmin = INT32_MAX, jmax = INT32_MIN;
-            for (; q < info.size() && h.patches[q].level == L; ++q) {
-                imin = std::min(imin, h.patches[q].i0 / h.P); imax = std::max(imax, h.patches[q].i0 / h.P);
-                jmin = std::min(jmin, h.patches[q].j0 / h.P); jmax = std::max(jmax, h.patches[q].j0 / h.P);
+            for (int32_t r : m) {
+                imin = std::min(imin, h.patches[size_t(r)].i0 / h.P); imax = std::max(imax, h.patches[size_t(r)].i0 / h.P);
+                jmin = std::min(jmin, h.patches[size_t(r)].j0 / h.P); jmax = std::max(jmax, h.patches[size_t(r)].j0 / h.P);
             }
             PatchLevel &l = lev[size_t(L)];
-            if (l.n != 0) { ok = false; break; }                          // patches not sorted by level: no map
-            l = PatchLevel{int32_t(p), int32_t(q - p), imin, jmin, imax - imin + 1, jmax - jmin + 1,
-                           int32_t(map_total), info[p].cw};
+            l = PatchLevel{m.front(), int32_t(m.size()), imin, jmin, imax - imin + 1, jmax - jmin + 1,
+                           int32_t(map_total), info[size_t(m.front())].cw};
             map_total += int64_t(l.npx) * l.npy;
             if (map_total > (int64_t(1) << 26)) { ok = false; break; }
             pmap.resize(size_t(map_total), -1);
-            for (size_t r = p; r < q; ++r)
-                pmap[size_t(l.map_off) + size_t(h.patches[r].j0 / h.P - jmin) * l.npx + (h.patches[r].i0 / h.P - imin)] = int32_t(r);
-            p = q;
+            for (int32_t r : m)
+                pmap[size_t(l.map_off) + size_t(h.patches[size_t(r)].j0 / h.P - jmin) * l.npx + (h.patches[size_t(r)].i0 / h.P - imin)] = r;
         }
         // groups of 8 target patches in sorted order with their offset boxes.  List 0 (any patches of a level) serves
         // the pair classes "same level" and "finer source"; lists 1 / 2 (patches of one residue class of (pi, pj)
@@ -244,7 +244,7 @@ bool build_patch_plan(sg_ctx *c) {
                 for (int cls = 0; cls < F * F && ok; ++cls) {
                     const int cx = cls % F, cy = cls / F;
                     std::vector<int32_t> members;
-                    for (int32_t r = l.p0; r < l.p0 + l.n; ++r)
+                    for (int32_t r : of_level[size_t(L)])
                         if ((h.patches[size_t(r)].i0 / h.P) % F == cx && (h.patches[size_t(r)].j0 / h.P) % F == cy)
                             members.push_back(r);
                     // 8 consecutive members should be a compact 4 x 2 block of the class's own patch lattice (pitch F):

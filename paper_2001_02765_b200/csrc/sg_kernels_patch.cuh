@@ -10,8 +10,8 @@ struct PatchInfo {                    // one leaf patch on the integer lattice
     int32_t level;
 };
 
-struct PatchLevel {                   // the leaf patches of one level (contiguous in the sorted patch list)
-    int32_t p0, n;                    // patches [p0, p0 + n)
+struct PatchLevel {                   // the leaf patches of one level (the patch list may be in any order)
+    int32_t p0, n;                    // first patch of the level in the list, number of patches
     int32_t pimin, pjmin, npx, npy;   // bounding box of their positions in patch units (i0 / P, j0 / P)
     int32_t map_off;                  // pmap[map_off + (pj - pjmin) * npx + (pi - pimin)] = patch index or -1
     int32_t cw;                       // cell width in lattice units

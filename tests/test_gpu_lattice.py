@@ -173,6 +173,23 @@ def test_four_level_gradient_refined_layout_at_scale(torch_cuda):
     check(gx[idx], gy[idx], ox, oy)
 
 
+def test_patch_order_invariance_in_lattice_mode(torch_cuda):
+    """The patch list may come in any order (levels interleaved): the offset-table plan is built per level from the
+    patches wherever they are in the list; permuting the list permutes the output."""
+    lay = random_refined_layout(4, 6, 16, 3, 0.3)
+    sigma = _noisy_kuzmin(lay, 44)
+    PP = lay.P * lay.P
+    perm = np.random.default_rng(3).permutation(lay.n_patches)
+    lay2 = Layout(lay.n_levels, lay.cell_width, lay.x0, lay.y0, lay.P, lay.patches[perm].copy())
+    sig2 = sigma.reshape(-1, PP)[perm].reshape(-1)
+    fx, fy = gpu_force(torch_cuda, lay, sigma, "lattice_blocked")
+    gx, gy = gpu_force(torch_cuda, lay2, sig2, "lattice_blocked")
+    s = max(np.abs(fx).max(), np.abs(fy).max())
+    assert np.abs(gx.reshape(-1, PP) - fx.reshape(-1, PP)[perm]).max() <= 1e-13 * s
+    assert np.abs(gy.reshape(-1, PP) - fy.reshape(-1, PP)[perm]).max() <= 1e-13 * s
+    check(gx, gy, *oracle_force(lay2, sig2, np.arange(lay2.n_cells)))
+
+
 def test_unsupported_patch_size_is_refused(torch_cuda):
     from paper_2001_02765_b200 import SgDisk, SgError, binding
     lay = paper_ilr_layout(32, 2)                                  # P = 1 quadtree

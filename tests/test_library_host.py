@@ -143,7 +143,7 @@ def _near_pair_counts(lay):
             int(sum(cnt[l] * cnt[l - 2] for l in range(2, L))), int(sum(cnt[l] * cnt[l + 2] for l in range(L - 2)))]
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4", "nest5", "rand1", "rand2", "rand3", "gap"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4", "nest5", "rand1", "rand2", "rand3", "gap", "shuffled"])
 def test_lattice_plan_reaches_every_near_patch_pair_exactly_once(name):
     """Host replay of the walk of the offset-table kernels (groups x offsets x warps, the same index arithmetic as
     patch_offset_kernel): every patch pair at most two levels apart is reached exactly once, in the right class."""
@@ -155,6 +155,10 @@ def test_lattice_plan_reaches_every_near_patch_pair_exactly_once(name):
         lay = Layout(3, np.array([1.0, 0.5, 0.25]), 0.0, 0.0, 16,
                      _sorted_patches([(0, 16, 0), (0, 0, 16), (0, 16, 16)] +
                                      [(2, 16 * i, 16 * j) for j in range(4) for i in range(4)]))
+    elif name == "shuffled":                                       # patch list in random order, levels interleaved
+        lay = random_refined_layout(5, 7, 16, 4, 0.35)
+        lay = Layout(lay.n_levels, lay.cell_width, lay.x0, lay.y0, lay.P,
+                     lay.patches[np.random.default_rng(9).permutation(lay.n_patches)].copy())
     else:
         lay = random_refined_layout(int(name[4:]), 7, 16, 4, 0.35)
     with SgDisk.from_layout(lay, device=-1) as d:
