@@ -103,6 +103,9 @@ def test_layout_errors():
     with pytest.raises(SgError) as e:
         mk(P=0)
     assert e.value.code == binding.SG_ERR_ARG
+    with pytest.raises(SgError) as e:                  # empty patch list
+        SgDisk(1, [1.0], 0, 0, 16, np.zeros((0, 3), dtype=np.int32), device=-1)
+    assert e.value.code == binding.SG_ERR_ARG
     with pytest.raises(SgError) as e:                  # lattice too large for exact FP64 integers
         SgDisk(1, [1.0], 0, 0, 16, np.array([[0, 1 << 25, 0]], dtype=np.int32), device=-1)
     assert e.value.code == binding.SG_ERR_LAYOUT
