@@ -553,6 +553,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
         // an event recorded on the caller's stream and are joined back into it (capturable in a CUDA graph)
         double *part = c->dev.part;
         int n_launch = 0;
+        const bool debug_sync = std::getenv("SG_DEBUG_SYNC") != nullptr;   // debugging aid: name the failing launch
         auto on_stream = [&](int idx) -> cudaStream_t {
             if (idx == 0) return s;
             cudaStream_t st = c->side[size_t(idx - 1)];
@@ -576,6 +577,13 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
                 if (po.variant[v]) {
                     launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, on_stream(n_launch++));
                     part += int64_t(po.n_split) * 2 * c->count;
+                    if (debug_sync) {
+                        const cudaError_t e = cudaDeviceSynchronize();
+                        if (e != cudaSuccess) {
+                            c->err = "patch_offset_kernel<" + std::to_string(v) + ">: " + cudaGetErrorString(e);
+                            return SG_ERR_CUDA;
+                        }
+                    }
                 }
         if (!blocked || far)
             launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 3 : 0, on_stream(n_launch++));

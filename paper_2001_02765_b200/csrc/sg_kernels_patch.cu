@@ -210,11 +210,13 @@ struct OffCls {
     static constexpr int TBUF = ROWS * TROW;
     static constexpr bool DB = F < 4;                                     // double-buffered tables (two CTAs per SM)
     static constexpr int LDIST = coarser ? -(F == 2 ? 1 : 2) : finer ? (F == 2 ? 1 : 2) : 0;   // source level - target level
-    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16 + size_t(kOffWarps) * kBlkW * 8;
+    static constexpr bool WG = F == 4;                                    // weights straight from global / L1: the table
+                                                                          // leaves no room for weight buffers at 2 CTAs per SM
+    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16 + (WG ? 0 : size_t(kOffWarps) * kBlkW * 8);
 };
 
 template <int V>
-__global__ void __launch_bounds__(kOffWarps * 32, (OffCls<V>::DB ? 2 : 1))
+__global__ void __launch_bounds__(kOffWarps * 32, 2)
 patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
                     const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int n_groups,
@@ -234,7 +236,8 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int l = lane & 15, h = lane >> 4;
 
-    for (int i = tid; i < kOffWarps * kBlkW; i += kOffWarps * 32) sW[i] = 0.0;           // the padding stays zero
+    if (!C::WG)
+        for (int i = tid; i < kOffWarps * kBlkW; i += kOffWarps * 32) sW[i] = 0.0;       // the padding stays zero
     double *W = sW + warp * kBlkW;
 
     const int n_items = n_groups * n_split;
@@ -307,16 +310,18 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         auto consume = [&](int b, const double2 *T) {
             // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
             const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride);
-            __syncwarp();
+            if (!C::WG) {
+                __syncwarp();
 #pragma unroll
-            for (int q = 0; q < 5; ++q) {
-                const int e2 = lane + 32 * q;
-                if (e2 < 17 * 9) {
-                    const int j = e2 / 9, c2 = e2 - 9 * j;
-                    *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
+                for (int q = 0; q < 5; ++q) {
+                    const int e2 = lane + 32 * q;
+                    if (e2 < 17 * 9) {
+                        const int j = e2 / 9, c2 = e2 - 9 * j;
+                        *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
+                    }
                 }
+                __syncwarp();
             }
-            __syncwarp();
             // entry (row, col) = (j RB - l RA + MMIN, i RB - k RA + MMIN) for vertex (i, j) and target (k, l)
             if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;   // column F t + this - cc
             else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
@@ -329,7 +334,8 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
 #pragma unroll
                 for (int t = 0; t < NT; ++t) {
                     if ((t & 1) == 0 && t <= P) {                         // vertices t, t+1 (column 17 is zero padding)
-                        const double2 w2 = *reinterpret_cast<const double2 *>(wrow + t);
+                        const double2 w2 = C::WG ? __ldg(src + j * 9 + t / 2)           // warp-uniform address: L1 broadcast
+                                                 : *reinterpret_cast<const double2 *>(wrow + t);
                         wv[t] = w2.x;
                         wv[t + 1] = w2.y;
                     }
@@ -410,7 +416,7 @@ void launch_patch_offset_one(const DevLayout &d, const PatchArrays &pa, const Of
     if (n_groups == 0) return;
     const PatchGroup *groups = pa.groups;
     for (int q = 0; q < list; ++q) groups += po.n_groups[q];
-    const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(OffCls<V>::DB ? 2 : 1) * sms));
+    const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(2) * sms));
     patch_offset_kernel<V><<<grid, kOffWarps * 32, OffCls<V>::smem, s>>>(
         pa.info, pa.levels, groups, pa.pmap, pa.wQ, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,
         po.last_patch, first, count, part, d.queue + 1 + V, kLogKeepMask);
