@@ -112,6 +112,8 @@ int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx
  * like one piece of work on cuda_stream (and can be captured in a CUDA graph after one warm-up call).
  * Test aid: with the environment variable SG_POISON_PARTIALS set, the internal partial-sum buffer is filled
  * with NaN when it is (re)allocated, so that a partial sum no kernel wrote would surface in Fx, Fy.
+ * Debugging aid: with SG_DEBUG_SYNC set, lattice mode synchronises after every pair-class launch and names the one
+ * that failed in sg_last_error (it serialises the launches; not for timing).
  */
 int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
 
