@@ -124,16 +124,26 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
                     }
                 }
             } else {
+                // far pair: every (target, vertex) pair directly, column by column as in interaction_kernel: u, u^2 and
+                // s(u) once per column, v by exact integer steps, 21 FP64-pipe instructions per pair
                 __syncthreads();
-                const double *wrow = sw;
-                for (int j = 0; j <= P; ++j, wrow += P + 1) {
-                    const double v = double(B.Y0 + j * B.cw - yt);
-#pragma unroll 2
-                    for (int i = 0; i <= P; ++i) {
-                        const double2 T = pair_terms(double(B.X0 + i * B.cw - xt), v, tabb, keep);
-                        ax = fma(wrow[i], T.x, ax);
-                        ay = fma(wrow[i], T.y, ay);
+                const double dv = double(B.cw), v0 = double(B.Y0 - yt);
+                for (int i = 0; i <= P; ++i) {
+                    const double u = double(B.X0 + i * B.cw - xt), uu = u * u, au = fabs(u);
+                    double cy = 0.0, v = v0;
+#pragma unroll 4
+                    for (int j = 0; j <= P; ++j, v += dv) {
+                        const double w = sw[j * (P + 1) + i];
+                        const double q = fma(v, v, uu);
+                        const double y0 = rsqrt_approx(q);
+                        const double t = q * y0;
+                        const double e = fma(-t, y0, 1.0);
+                        const double pp = fma(0.375, e, 0.5);
+                        const double r = fma(t, pp * e, t);
+                        ax = fma(w, flip_sign_by(fast_ln(fabs(v) + r, tabb, keep), v), ax);
+                        cy = fma(w, fast_ln(au + r, tabb, keep), cy);
                     }
+                    ay += flip_sign_by(cy, u);
                 }
             }
         }
