@@ -190,6 +190,42 @@ def test_patch_order_invariance_in_lattice_mode(torch_cuda):
     check(gx, gy, *oracle_force(lay2, sig2, np.arange(lay2.n_cells)))
 
 
+def test_fuzz_random_hierarchies_lattice_vs_direct(torch_cuda):
+    """Seeded random hierarchies (1-5 levels, 2-8 base patches per side, random refinement fraction, every third
+    patch list shuffled, every other case a random target slice): lattice mode vs the direct kernel on one context,
+    plan check, all outputs finite with NaN-poisoned partial sums."""
+    from paper_2001_02765_b200 import SgDisk
+    rng = np.random.default_rng(123)
+    worst = 0.0
+    for case in range(16):
+        n0, nl, frac = int(rng.integers(2, 9)), int(rng.integers(1, 6)), float(rng.uniform(0.1, 0.7))
+        lay = random_refined_layout(1000 + case, n0, 16, nl, frac)
+        if case % 3 == 0:
+            lay = Layout(lay.n_levels, lay.cell_width, lay.x0, lay.y0, lay.P,
+                         lay.patches[rng.permutation(lay.n_patches)].copy())
+        sigma = _noisy_kuzmin(lay, 500 + case)
+        first, count = 0, lay.n_cells
+        if case % 2:
+            first = int(rng.integers(0, lay.n_cells))
+            count = int(rng.integers(1, lay.n_cells - first + 1))
+        with SgDisk.from_layout(lay, device=0) as d:
+            chk = d.lattice_plan_check()
+            assert chk["duplicates"] == 0 and chk["wrong_level"] == 0 and chk["patches_missing_from_launched_lists"] == 0
+            d.set_density(torch_cuda.as_tensor(sigma).cuda())
+            d.set_target_range(first, count)
+            out = {}
+            for mode in ("direct", "lattice"):
+                d.set_interaction_mode(mode)
+                Fx, Fy = d.force()
+                torch_cuda.cuda.synchronize()
+                out[mode] = (Fx.cpu().numpy(), Fy.cpu().numpy())
+        (ax, ay), (bx, by) = out["direct"], out["lattice"]
+        assert np.all(np.isfinite(bx)) and np.all(np.isfinite(by)), case
+        s = max(np.abs(ax).max(), np.abs(ay).max())
+        worst = max(worst, max(np.abs(ax - bx).max(), np.abs(ay - by).max()) / s)
+    assert worst <= 1e-12, worst
+
+
 def test_unsupported_patch_size_is_refused(torch_cuda):
     from paper_2001_02765_b200 import SgDisk, SgError, binding
     lay = paper_ilr_layout(32, 2)                                  # P = 1 quadtree
