@@ -109,9 +109,12 @@ int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx
  * (no floating-point atomics).  SG_ERR_STATE if no density has been set.  In SG_MODE_LATTICE on a
  * multi-level layout the independent pair-class kernels run on side streams owned by the context,
  * forked from and joined back into cuda_stream by events, so for the caller the call still orders
- * like one piece of work on cuda_stream (and can be captured in a CUDA graph after one warm-up call).
+ * like one piece of work on cuda_stream (and can be captured in a CUDA graph; a launch error after the fork
+ * still joins the side streams before SG_ERR_CUDA is returned).  The caller's current device is left unchanged.
+ * The call enqueues kernel launches (and event records / waits) only: the internal partial-sum buffer is sized by
+ * sg_create, sg_set_interaction_mode, sg_set_target_range and the first sg_set_density_linear, all host-synchronous.
  * Test aid: with the environment variable SG_POISON_PARTIALS set, the internal partial-sum buffer is filled
- * with NaN when it is (re)allocated, so that a partial sum no kernel wrote would surface in Fx, Fy.
+ * with NaN on cuda_stream at the start of every sg_force, so that a partial sum no kernel wrote surfaces in Fx, Fy.
  * Debugging aid: with SG_DEBUG_SYNC set, lattice mode synchronises after every pair-class launch and names the one
  * that failed in sg_last_error (it serialises the launches; not for timing).
  */
@@ -142,44 +145,6 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 #define SG_MODE_LATTICE 1
 #define SG_MODE_LATTICE_BLOCKED 2
 int sg_set_interaction_mode(sg_ctx *ctx, int mode);
-
-/*
- * Diagnostic of the SG_MODE_LATTICE launch plan (P = 16), computed on the host (works on a context created with
- * device < 0): replays the walk of the offset-table kernels over every target group and patch offset and counts
- * the (target patch, source patch) pairs it reaches.  out[16]:
- *   out[0..4]  pairs reached per pair class: same level, source one level coarser, one finer, two coarser, two finer
- *   out[5]     pairs reached more than once (must be 0)      out[6]  pairs of the wrong level distance (must be 0)
- *   out[7..9]  target groups in the three group lists         out[10] offsets visited (= offset tables at most)
- *   out[11]    1 if the plan exists (P = 16, patch maps fit), else 0 and everything else is 0
- *   out[12]    target patches that are not exactly once in a group list whose pair classes are launched (must be 0:
- *              every launched class writes the partial sums of every target)      out[13..15] reserved, 0
- * Every patch pair at most two levels apart must be reached exactly once; pairs farther apart are summed directly.
- * Only for layouts of at most 65,536 patches (larger: counts stay 0).
- */
-int sg_lattice_plan_check(const sg_ctx *ctx, int64_t *out);
-
-/* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
-int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
-
-/*
- * Kernel timing for the roofline line.  While enabled, every sg_force records a pair of CUDA events
- * on the caller's stream around the interaction kernel (S3) only; no synchronisation is added to
- * sg_force.  sg_get_kernel_times synchronises on the newest end event and returns the durations (ms)
- * of the sg_force calls made since timing was enabled, oldest first; at most 64 are kept.
- *   ms: host [capacity];  n: host, receives the number written.
- */
-int sg_set_kernel_timing(sg_ctx *ctx, int enable);
-int sg_get_kernel_times(sg_ctx *ctx, float *ms, int capacity, int *n);
-
-/* FP64-pipe instructions (warp-level, per (target, vertex) pair) and FP64 FLOPs per pair of the
- * interaction kernel as built (counted from its SASS); vertex evaluations per
- * sg_force with the current target range.  Any pointer may be NULL. */
-int sg_kernel_model(const sg_ctx *ctx, double *fp64_instr_per_pair, double *flops_per_pair,
-                    double *pair_evaluations);
-
-/* Diagnostic: sustained DFMA rate of the device (8 independent chains per thread, full occupancy),
- * in FP64 TFLOP/s (FMA = 2), and the same as warp-instructions/s.  Synchronous. */
-int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s);
 
 const char *sg_last_error(const sg_ctx *ctx);        /* ctx may be NULL: error of the last failed sg_create */
 const char *sg_version(void);

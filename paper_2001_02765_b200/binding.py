@@ -1,4 +1,4 @@
-"""ctypes binding of include/sg_disk.h -- same names, argument marshalling only.
+"""ctypes binding of include/sg_disk.h and include/sg_disk_diag.h -- same names, argument marshalling only.
 
 PyTorch is used for device memory and streams: sigma / Fx / Fy are CUDA float64 tensors whose
 ``data_ptr()`` is handed to the C ABI, and work is enqueued on torch's current stream.
@@ -17,11 +17,11 @@ SG_OK, SG_ERR_ARG, SG_ERR_LAYOUT, SG_ERR_CUDA, SG_ERR_STATE = 0, -1, -2, -3, -4
 _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_CUDA: "SG_ERR_CUDA",
               SG_ERR_STATE: "SG_ERR_STATE"}
 
-# every symbol include/sg_disk.h declares (tests check the header and this list agree)
+# every symbol include/sg_disk.h and include/sg_disk_diag.h declare (tests check the headers and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
     "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
-    "sg_kernel_model", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
+    "sg_kernel_model", "sg_kernel_instruction_counts", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
 
@@ -86,7 +86,9 @@ def load_library():
     lib.sg_get_kernel_times.restype = c_int
     lib.sg_get_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), c_int, ctypes.POINTER(c_int)]
     lib.sg_kernel_model.restype = c_int
-    lib.sg_kernel_model.argtypes = [vp, dp, dp, dp]
+    lib.sg_kernel_model.argtypes = [vp, dp, dp, dp, dp]
+    lib.sg_kernel_instruction_counts.restype = c_int
+    lib.sg_kernel_instruction_counts.argtypes = [c_int, dp, dp]
     lib.sg_measure_fp64_peak.restype = c_int
     lib.sg_measure_fp64_peak.argtypes = [c_int, dp, dp]
     lib.sg_last_error.restype = ctypes.c_char_p
@@ -99,6 +101,16 @@ def load_library():
 
 def version() -> str:
     return load_library().sg_version().decode()
+
+
+def kernel_instruction_counts(kernel: int):
+    """(FP64-pipe instructions, FLOPs) per (target, vertex) pair of the direct (0) or slope (1) kernel as built."""
+    lib = load_library()
+    a, b = ctypes.c_double(), ctypes.c_double()
+    rc = lib.sg_kernel_instruction_counts(int(kernel), ctypes.byref(a), ctypes.byref(b))
+    if rc != SG_OK:
+        raise SgError(rc, "unknown kernel id")
+    return a.value, b.value
 
 
 def measure_fp64_peak(device: int = 0):
@@ -114,9 +126,9 @@ def measure_fp64_peak(device: int = 0):
 from .sharding import shard_range  # noqa: E402,F401  (re-exported: one definition of the partition)
 
 
-def _stream_ptr():
+def _stream_ptr(device: int):
     import torch
-    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
 
 
 class SgDisk:
@@ -187,7 +199,7 @@ class SgDisk:
     def set_density(self, sigma):
         """sigma: CUDA float64 tensor [N] in library cell order (asynchronous on the current stream)."""
         self._require_cuda(sigma, self.num_cells, "sigma")
-        self._check(self._lib.sg_set_density(self._ctx, ctypes.c_void_p(sigma.data_ptr()), _stream_ptr()))
+        self._check(self._lib.sg_set_density(self._ctx, ctypes.c_void_p(sigma.data_ptr()), _stream_ptr(self.device)))
 
     def set_density_linear(self, sigma, dx, dy):
         """sigma, dx, dy: CUDA float64 tensors [N] (value and physical slopes of Eq. 6 per leaf); the next
@@ -196,7 +208,7 @@ class SgDisk:
             self._require_cuda(t, self.num_cells, name)
         self._check(self._lib.sg_set_density_linear(self._ctx, ctypes.c_void_p(sigma.data_ptr()),
                                                     ctypes.c_void_p(dx.data_ptr()), ctypes.c_void_p(dy.data_ptr()),
-                                                    _stream_ptr()))
+                                                    _stream_ptr(self.device)))
 
     def set_target_range(self, first: int, count: int):
         self._check(self._lib.sg_set_target_range(self._ctx, int(first), int(count)))
@@ -226,7 +238,7 @@ class SgDisk:
         self._require_cuda(Fx, self._count, "Fx")
         self._require_cuda(Fy, self._count, "Fy")
         self._check(self._lib.sg_force(self._ctx, ctypes.c_void_p(Fx.data_ptr()), ctypes.c_void_p(Fy.data_ptr()),
-                                       _stream_ptr()))
+                                       _stream_ptr(self.device)))
         return Fx, Fy
 
     def launch_counts(self):
@@ -244,9 +256,11 @@ class SgDisk:
         return [float(buf[i]) for i in range(n.value)]
 
     def kernel_model(self) -> dict:
-        a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
-        self._check(self._lib.sg_kernel_model(self._ctx, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
-        return dict(fp64_instr_per_pair=a.value, flops_per_pair=b.value, pair_evaluations=c.value)
+        a, b, c, e = ctypes.c_double(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        self._check(self._lib.sg_kernel_model(self._ctx, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c),
+                                              ctypes.byref(e)))
+        return dict(fp64_instr_per_pair=a.value, flops_per_pair=b.value, pair_evaluations=c.value,
+                    executed_evaluations=e.value)
 
     def _require_cuda(self, t, n, name):
         import torch

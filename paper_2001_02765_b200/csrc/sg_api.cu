@@ -11,6 +11,7 @@
 #include "sg_kernels_lin.cuh"
 #include "sg_kernels_patch.cuh"
 #include "sg_layout.h"
+#include "../../include/sg_disk_diag.h"
 
 using namespace sg;
 
@@ -60,6 +61,17 @@ namespace {
         }                                                                               \
     } while (0)
 
+// The library works on the context's device and leaves the caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        err = cudaSetDevice(device);
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 template <class T>
 int dev_alloc(sg_ctx *c, T **p, int64_t n) {
     const size_t bytes = size_t(std::max<int64_t>(n, 1)) * sizeof(T);
@@ -79,12 +91,12 @@ int upload(sg_ctx *c, T **p, const std::vector<T> &h) {
 
 // Work items = target blocks x source splits, pulled from an atomic queue by a persistent grid of
 // 2 CTAs per SM (about 16 items per CTA).  Pick the split count that keeps the last round fullest.
-ForcePlan make_plan(const sg_ctx *c) {
+ForcePlan make_plan(const sg_ctx *c, bool linear) {
     ForcePlan p;
     p.first = c->first; p.count = c->count;
-    p.smem = c->linear ? interaction_lin_smem_bytes(c->dev.tab_entries) : interaction_smem_bytes(c->dev.tab_entries);
+    p.smem = linear ? interaction_lin_smem_bytes(c->dev.tab_entries) : interaction_smem_bytes(c->dev.tab_entries);
     if (p.count == 0) return p;
-    p.T = c->linear ? lin_targets_per_thread() : (p.count > 16384 ? 4 : 1);
+    p.T = linear ? lin_targets_per_thread() : (p.count > 16384 ? 4 : 1);
     const int64_t per_block = int64_t(kThreads) * p.T;
     p.n_tblocks = int((p.count + per_block - 1) / per_block);
     const int slots = c->sm_count * 2;
@@ -106,9 +118,20 @@ ForcePlan make_plan(const sg_ctx *c) {
     return p;
 }
 
-int ensure_partials(sg_ctx *c, const ForcePlan &p) {
-    const int64_t need = int64_t(p.n_split) * 2 * p.count;
+// The partial-sum buffer [n_split][2][count].  It is sized by reserve_partials() from the host-synchronous calls that
+// change the plan (sg_create, sg_set_interaction_mode, sg_set_target_range, the first sg_set_density_linear), so that
+// sg_force itself never allocates or synchronises (CUDA-graph capture).  grow_partials is the fallback for
+// a plan nobody announced: refused during stream capture (a captured graph would keep the freed pointer).
+int grow_partials(sg_ctx *c, int64_t need, cudaStream_t capturing_on) {
     if (need <= c->dev.part_capacity) return SG_OK;
+    if (capturing_on != nullptr || c->dev.part) {
+        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(capturing_on, &st) == cudaSuccess && st != cudaStreamCaptureStatusNone) {
+            c->err = "sg_force during stream capture needs a larger partial-sum buffer: call sg_force once with the same "
+                     "mode and target range before capturing";
+            return SG_ERR_STATE;
+        }
+    }
     if (c->dev.part) {
         SG_CUDA(c, cudaDeviceSynchronize());
         cudaFree(c->dev.part);
@@ -119,9 +142,6 @@ int ensure_partials(sg_ctx *c, const ForcePlan &p) {
     int rc = dev_alloc(c, &c->dev.part, need);
     if (rc) return rc;
     c->dev.part_capacity = need;
-    // test aid (tests/conftest.py sets it): NaN-fill the partial sums, so that a slot no kernel writes shows up in the
-    // forces instead of passing as a lucky zero of fresh device memory
-    if (std::getenv("SG_POISON_PARTIALS")) SG_CUDA(c, cudaMemset(c->dev.part, 0xFF, size_t(need) * sizeof(double)));
     return SG_OK;
 }
 
@@ -143,7 +163,7 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
     return pp;
 }
 
-// Blocked kernels (patch pairs at most one level apart): one work item = (group of <= 8 target patches, split of the
+// Blocked kernels (patch pairs at most two levels apart): one work item = (group of <= 8 target patches, split of the
 // group's offset box), per pair class.
 int offset_classes(const OffsetPlan &po) {
     int n = 0;
@@ -182,9 +202,44 @@ OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
     return po;
 }
 
-// P = 16: the register-blocked offset-table kernels (measured faster than the generic kernel at every size,
-// cfg 1: 25 vs 37 us, cfg 3: 2.6 vs 4.0 ms); P = 8: generic kernel
+// P = 16: the register-blocked offset-table kernels for pairs <= 2 levels apart (measured faster than the generic
+// kernel at every size, cfg 1: 25 vs 37 us, cfg 3: 2.6 vs 4.0 ms), the generic kernel only for the direct sum of
+// the pairs >= 3 levels apart; P = 8: generic kernel (tables for pairs <= 1 level apart, direct sum beyond)
 bool use_blocked(const sg_ctx *c, const PatchPlan &) { return c->patch.blocked; }
+
+// Everything one sg_force launches with the current mode and target range.
+struct StepPlan {
+    ForcePlan p;                           // direct / slope kernel, and the finalise kernel (p.n_split partial sums per target)
+    PatchPlan pp;                          // generic kernel: everything (P = 8) or the pairs >= 3 levels apart (P = 16)
+    OffsetPlan po;                         // blocked kernels: pairs at most two levels apart
+    bool by_patch = false, blocked = false, far = true;
+    int64_t partials() const { return int64_t(p.n_split) * 2 * p.count; }
+};
+
+StepPlan make_step_plan(const sg_ctx *c, bool linear) {
+    StepPlan sp;
+    sp.p = make_plan(c, linear);
+    sp.by_patch = c->use_patch && !linear;
+    if (sp.by_patch) {
+        sp.pp = make_patch_plan(c);
+        sp.blocked = use_blocked(c, sp.pp);
+        if (sp.blocked) {
+            sp.po = make_offset_plan(c, sp.pp);
+            sp.far = c->host.n_levels > 3;                     // pairs >= 3 levels apart exist only then
+            sp.p.n_split = offset_classes(sp.po) * sp.po.n_split + (sp.far ? sp.pp.n_split : 0);
+        } else {
+            sp.p.n_split = sp.pp.n_split;
+        }
+    }
+    return sp;
+}
+
+// Called from the host-synchronous calls that change the plan: the buffer fits the zeroth-order and the slope path.
+int reserve_partials(sg_ctx *c) {
+    if (c->device < 0) return SG_OK;
+    const int64_t need = std::max(make_step_plan(c, false).partials(), make_step_plan(c, true).partials());
+    return grow_partials(c, need, nullptr);
+}
 
 // Host-side plan of the offset-table kernels (P = 16): per-patch lattice info, per-level dense patch maps, target
 // groups with their offset boxes per pair class.  No CUDA: also built for host-only contexts (sg_lattice_plan_check).
@@ -413,13 +468,15 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
         c->first = 0; c->count = c->host.N;
         c->patch_plan_ok = build_patch_plan(c);
         if (device >= 0) {
-            cudaError_t e = cudaSetDevice(device);
+            DeviceGuard guard(device);
+            cudaError_t e = guard.err;
             if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
             if (e != cudaSuccess) {
                 c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(e);
                 rc = SG_ERR_CUDA;
             } else {
                 rc = upload_layout(c);
+                if (rc == SG_OK) rc = reserve_partials(c);
             }
         }
     }
@@ -435,7 +492,7 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
 void sg_destroy(sg_ctx *c) {
     if (!c) return;
     if (c->device >= 0) {
-        cudaSetDevice(c->device);
+        DeviceGuard guard(c->device);
         cudaDeviceSynchronize();
         for (void *p : c->allocs) cudaFree(p);
         for (cudaEvent_t e : c->ev0) cudaEventDestroy(e);
@@ -477,7 +534,8 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     if (!sigma_dev) { c->err = "sigma_dev is NULL"; return SG_ERR_ARG; }
     if (c->device < 0) { c->err = "host-only context (device < 0): no CUDA path, and there is no CPU fallback"; return SG_ERR_CUDA; }
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    SG_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
     launch_vertex_weights(c->dev, sigma_dev, s);
     launch_line_tables(c->dev, s);
     if (c->patch.enabled) launch_patch_weights(c->patch, sigma_dev, s);
@@ -493,7 +551,8 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
     if (!sigma_dev || !dx_dev || !dy_dev) { c->err = "sigma_dev / dx_dev / dy_dev is NULL"; return SG_ERR_ARG; }
     if (c->device < 0) { c->err = "host-only context (device < 0): no CUDA path, and there is no CPU fallback"; return SG_ERR_CUDA; }
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    SG_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
     LinArrays &l = c->lin;
     if (!l.allocated) {
         const HostLayout &h = c->host;
@@ -510,6 +569,7 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
         if ((rc = dev_alloc(c, &l.TBy3, int64_t(d.ntX) * d.nY * 3))) return rc;
         SG_CUDA(c, configure_lin_kernels(d.tab_entries));
         l.allocated = true;
+        if ((rc = reserve_partials(c))) return rc;
     }
     launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
     SG_CUDA(c, cudaGetLastError());
@@ -525,42 +585,27 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (c->count == 0) return SG_OK;
     if (!Fx_dev || !Fy_dev) { c->err = "Fx_dev / Fy_dev is NULL"; return SG_ERR_ARG; }
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    SG_CUDA(c, cudaSetDevice(c->device));
-    ForcePlan p = make_plan(c);
-    const bool by_patch = c->use_patch && !c->linear;
-    PatchPlan pp;                          // generic kernel: everything (small problems) or pairs >= 2 levels apart
-    OffsetPlan po;                         // blocked kernels: pairs at most one level apart
-    bool blocked = false, far = true;
-    if (by_patch) {
-        pp = make_patch_plan(c);
-        blocked = use_blocked(c, pp);
-        if (blocked) {
-            po = make_offset_plan(c, pp);
-            far = c->host.n_levels > 3;
-            p.n_split = offset_classes(po) * po.n_split + (far ? pp.n_split : 0);  // finalise adds p.n_split partial sums per target
-        } else {
-            p.n_split = pp.n_split;
-        }
-    }
-    int rc = ensure_partials(c, p);
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
+    const StepPlan sp = make_step_plan(c, c->linear);
+    const ForcePlan &p = sp.p;
+    int rc = grow_partials(c, sp.partials(), s);           // no-op: reserve_partials() sized it (fallback otherwise)
     if (rc) return rc;
+    // test aid (tests/conftest.py sets it): NaN-fill the partial sums on the caller's stream before EVERY evaluation,
+    // so that a slot no kernel writes shows up in the forces instead of passing as the previous call's value
+    if (std::getenv("SG_POISON_PARTIALS"))
+        SG_CUDA(c, cudaMemsetAsync(c->dev.part, 0xFF, size_t(sp.partials()) * sizeof(double), s));
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
     if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
-    else if (by_patch) {
+    else if (sp.by_patch) {
         // every launch writes its own n_split slots of [2][count] partial sums and has its own work queue, so the
         // launches are independent: the first runs on the caller's stream, the others on side streams that wait for
         // an event recorded on the caller's stream and are joined back into it (capturable in a CUDA graph)
+        const OffsetPlan &po = sp.po;
         double *part = c->dev.part;
-        int n_launch = 0;
         const bool debug_sync = std::getenv("SG_DEBUG_SYNC") != nullptr;   // debugging aid: name the failing launch
-        auto on_stream = [&](int idx) -> cudaStream_t {
-            if (idx == 0) return s;
-            cudaStream_t st = c->side[size_t(idx - 1)];
-            cudaStreamWaitEvent(st, c->fork_ev, 0);
-            return st;
-        };
-        const int n_total = (blocked ? offset_classes(po) : 0) + ((!blocked || far) ? 1 : 0);
+        const int n_total = (sp.blocked ? offset_classes(po) : 0) + ((!sp.blocked || sp.far) ? 1 : 0);
         if (n_total > 1) {
             while (int(c->side.size()) < n_total - 1) {
                 cudaStream_t st; cudaEvent_t ev;
@@ -572,24 +617,45 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
             if (!c->fork_ev) SG_CUDA(c, cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
             SG_CUDA(c, cudaEventRecord(c->fork_ev, s));
         }
-        if (blocked)
+        // from here on a failure must still join the side streams back (a dangling fork would break a stream capture
+        // and leave the work queues undrained): remember the first error, keep going, join, then return it
+        cudaError_t first_err = cudaSuccess;
+        std::string where;
+        auto note = [&](cudaError_t e, const char *what) {
+            if (e != cudaSuccess && first_err == cudaSuccess) { first_err = e; where = what; }
+        };
+        int n_launch = 0;
+        auto on_stream = [&](int idx) -> cudaStream_t {
+            if (idx == 0) return s;
+            cudaStream_t st = c->side[size_t(idx - 1)];
+            note(cudaStreamWaitEvent(st, c->fork_ev, 0), "cudaStreamWaitEvent(fork)");
+            return st;
+        };
+        if (sp.blocked)
             for (int v = 0; v < kOffClasses; ++v)
                 if (po.variant[v]) {
-                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, on_stream(n_launch++));
+                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, c->sm_count, on_stream(n_launch));
+                    ++n_launch;
                     part += int64_t(po.n_split) * 2 * c->count;
-                    if (debug_sync) {
+                    if (debug_sync && first_err == cudaSuccess) {
                         const cudaError_t e = cudaDeviceSynchronize();
-                        if (e != cudaSuccess) {
-                            c->err = "patch_offset_kernel<" + std::to_string(v) + ">: " + cudaGetErrorString(e);
-                            return SG_ERR_CUDA;
-                        }
+                        if (e != cudaSuccess) { first_err = e; where = "patch_offset_kernel<" + std::to_string(v) + ">"; }
                     }
                 }
-        if (!blocked || far)
-            launch_patch_interaction(c->dev, c->patch, pp, c->first, c->count, part, blocked ? 3 : 0, on_stream(n_launch++));
+        if (!sp.blocked || sp.far) {
+            launch_patch_interaction(c->dev, c->patch, sp.pp, c->first, c->count, part, sp.blocked ? 3 : 0, on_stream(n_launch));
+            ++n_launch;
+        }
+        note(cudaGetLastError(), "pair-class kernel launch");
         for (int i = 1; i < n_launch; ++i) {
-            SG_CUDA(c, cudaEventRecord(c->join_ev[size_t(i - 1)], c->side[size_t(i - 1)]));
-            SG_CUDA(c, cudaStreamWaitEvent(s, c->join_ev[size_t(i - 1)], 0));
+            note(cudaEventRecord(c->join_ev[size_t(i - 1)], c->side[size_t(i - 1)]), "cudaEventRecord(join)");
+            note(cudaStreamWaitEvent(s, c->join_ev[size_t(i - 1)], 0), "cudaStreamWaitEvent(join)");
+        }
+        if (first_err != cudaSuccess) {
+            // the queues may be half drained: reset them so that the next call starts clean
+            cudaMemsetAsync(c->dev.queue, 0, kQueues * sizeof(unsigned int), s);
+            c->err = where + ": " + cudaGetErrorString(first_err);
+            return SG_ERR_CUDA;
         }
     }
     else launch_interaction(c->dev, p, s);
@@ -616,7 +682,10 @@ int sg_set_interaction_mode(sg_ctx *c, int mode) {
         return SG_ERR_ARG;
     }
     c->use_patch = mode != SG_MODE_DIRECT;
-    return SG_OK;
+    if (c->device < 0) return SG_OK;
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
+    return reserve_partials(c);
 }
 
 int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
@@ -625,7 +694,10 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
         c->err = "target range outside [0, N)"; return SG_ERR_ARG;
     }
     c->first = first; c->count = count;
-    return SG_OK;
+    if (c->device < 0) return SG_OK;
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
+    return reserve_partials(c);
 }
 
 int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
@@ -707,7 +779,8 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
 int sg_set_kernel_timing(sg_ctx *c, int enable) {
     if (!c) return SG_ERR_ARG;
     if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
-    SG_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
     if (enable && c->ev0.empty()) {
         c->ev0.resize(kTimingRing); c->ev1.resize(kTimingRing);
         for (int i = 0; i < kTimingRing; ++i) {
@@ -727,7 +800,8 @@ int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
     const int64_t have = std::min<int64_t>(c->timed_calls, kTimingRing);
     const int64_t take = std::min<int64_t>(have, capacity);
     if (take == 0) return SG_OK;
-    SG_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    SG_CUDA(c, guard.err);
     SG_CUDA(c, cudaEventSynchronize(c->ev1[(c->timed_calls - 1) % kTimingRing]));
     for (int64_t k = 0; k < take; ++k) {
         const int slot = int((c->timed_calls - take + k) % kTimingRing);
@@ -737,25 +811,39 @@ int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
     return SG_OK;
 }
 
-int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_per_pair, double *pair_evaluations) {
+int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_per_pair, double *pair_evaluations,
+                    double *executed_evaluations) {
     if (!c) return SG_ERR_ARG;
+    // algorithmic unit: one (target, deduplicated vertex) pair; one launch processes count * N_v
+    const double alg = double(c->count) * double(c->host.Nv);
+    if (pair_evaluations) *pair_evaluations = alg;
     if (c->use_patch && !c->linear) {
-        // lattice-offset path: one pair = (target, per-patch vertex) = 2 DFMA of the correlation; the offset tables
-        // ((2P)^2 pair-function evaluations per P^2 (P+1)^2 pairs, 1.4 % at P = 16) are not credited
-        const double nsrc = double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
+        // lattice-offset path: a pair costs the 2 DFMA of the correlation.  The kernels work on per-patch vertex
+        // sets, (P+1)^2 / P^2 more pairs than the deduplicated list: reported separately as executed work, not
+        // credited.  Not credited either: the offset tables and the pairs >= 3 levels apart that are summed
+        // directly (21 FP64 instructions each), so the algorithmic fraction is a lower bound on deep hierarchies.
         if (fp64_instr_per_pair) *fp64_instr_per_pair = 2.0;
         if (flops_per_pair) *flops_per_pair = 4.0;
-        if (pair_evaluations) *pair_evaluations = double(c->count) * nsrc;
+        if (executed_evaluations)
+            *executed_evaluations = double(c->count) * double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
         return SG_OK;
     }
     if (fp64_instr_per_pair) *fp64_instr_per_pair = c->linear ? kLinFp64InstrPerPair : kFp64InstrPerPair;
     if (flops_per_pair) *flops_per_pair = c->linear ? kLinFlopsPerPair : kFlopsPerPair;
-    if (pair_evaluations) *pair_evaluations = double(c->count) * double(c->host.Nv);   // algorithmic: real vertices
+    if (executed_evaluations) *executed_evaluations = double(c->count) * double(c->host.slot_vertex.size());   // incl. padding slots
+    return SG_OK;
+}
+
+int sg_kernel_instruction_counts(int kernel, double *fp64_instr_per_pair, double *flops_per_pair) {
+    if (kernel != 0 && kernel != 1) return SG_ERR_ARG;
+    if (fp64_instr_per_pair) *fp64_instr_per_pair = kernel ? kLinFp64InstrPerPair : kFp64InstrPerPair;
+    if (flops_per_pair) *flops_per_pair = kernel ? kLinFlopsPerPair : kFlopsPerPair;
     return SG_OK;
 }
 
 int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s) {
-    cudaError_t e = cudaSetDevice(device);
+    DeviceGuard guard(device);
+    cudaError_t e = guard.err;
     if (e == cudaSuccess) e = measure_dfma(tflops, warp_instr_per_s);
     if (e != cudaSuccess) { g_create_error = std::string("sg_measure_fp64_peak: ") + cudaGetErrorString(e); return SG_ERR_CUDA; }
     return SG_OK;

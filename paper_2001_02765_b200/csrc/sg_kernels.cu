@@ -275,10 +275,10 @@ size_t interaction_smem_bytes(int tab_entries) {
 }
 
 cudaError_t configure_kernels(int tab_entries) {
-    const int bytes = int(interaction_smem_bytes(tab_entries));
-    cudaError_t e = cudaFuncSetAttribute(interaction_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    const size_t bytes = interaction_smem_bytes(tab_entries);
+    cudaError_t e = opt_in_max_smem(interaction_kernel<4>, bytes);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(interaction_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return opt_in_max_smem(interaction_kernel<1>, bytes);
 }
 
 void launch_interaction(const DevLayout &d, const ForcePlan &p, cudaStream_t s) {

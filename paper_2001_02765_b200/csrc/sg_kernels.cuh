@@ -63,8 +63,27 @@ struct ForcePlan {
     size_t smem = 0;
 };
 
+// Opt-in dynamic shared memory.  cudaFuncAttributeMaxDynamicSharedMemorySize is a per-function, process-wide
+// setting, so it must not depend on the context that happens to be created last: every kernel gets the device's
+// maximum (opt-in limit minus the kernel's static shared memory), the same value whichever context asks.
+// `need_bytes` is what the asking context will launch with: cudaErrorInvalidValue if even the maximum is too small.
+template <class Kernel>
+inline cudaError_t opt_in_max_smem(Kernel kernel, size_t need_bytes) {
+    int dev = 0, optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, kernel);
+    if (e != cudaSuccess) return e;
+    const int max_dyn = optin - int(fa.sharedSizeBytes);
+    if (max_dyn < 0 || need_bytes > size_t(max_dyn)) return cudaErrorInvalidValue;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
+}
+
 size_t interaction_smem_bytes(int tab_entries);
-cudaError_t configure_kernels(int tab_entries);   // cudaFuncSetAttribute for the opt-in smem size
+cudaError_t configure_kernels(int tab_entries);   // opt-in smem (opt_in_max_smem) for the interaction kernels
 
 void launch_build_logtab(const DevLayout &d, cudaStream_t s);
 void launch_build_lnint(const DevLayout &d, cudaStream_t s);

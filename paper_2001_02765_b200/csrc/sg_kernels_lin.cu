@@ -226,8 +226,7 @@ size_t interaction_lin_smem_bytes(int tab_entries) {
 }
 
 cudaError_t configure_lin_kernels(int tab_entries) {
-    return cudaFuncSetAttribute(interaction_lin_kernel<kLinT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(interaction_lin_smem_bytes(tab_entries)));
+    return opt_in_max_smem(interaction_lin_kernel<kLinT>, interaction_lin_smem_bytes(tab_entries));
 }
 
 void launch_interaction_lin(const DevLayout &d, const LinArrays &l, const ForcePlan &p, cudaStream_t s) {

@@ -30,6 +30,6 @@ void launch_finalise_lin(const DevLayout &d, const LinArrays &l, const ForcePlan
 
 // per (target, vertex) pair: 22 DFMA + 3 DADD + 3 DMUL (+ 5 per (target, chunk)); see sg_kernels_lin.cu
 constexpr double kLinFp64InstrPerPair = 28.0 + 5.0 / kChunk;
-constexpr double kLinFlopsPerPair = 22 * 2 + 3 + 3 + 8.0 / kChunk;
+constexpr double kLinFlopsPerPair = 22 * 2 + 3 + 3 + 6.0 / kChunk;   // per chunk: 1 DFMA + 3 DADD + 1 DMUL
 
 }  // namespace sg

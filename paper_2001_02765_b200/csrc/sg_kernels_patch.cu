@@ -87,6 +87,8 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 
     const int n_items = n_tpatches * n_split;
     while (true) {
+        __syncthreads();           // every thread has read s_item of the previous item (an item whose source patches
+                                   // are all skipped runs no other barrier) and is done with sw / stab2
         if (tid == 0) s_item = int(atomicAdd(queue, 1u));
         __syncthreads();
         const int item = s_item;
@@ -405,8 +407,7 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
 
 template <int V>
 cudaError_t configure_patch_offset_one() {
-    return cudaFuncSetAttribute(patch_offset_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(OffCls<V>::smem));
+    return opt_in_max_smem(patch_offset_kernel<V>, OffCls<V>::smem);
 }
 
 cudaError_t configure_patch_offset() {
@@ -433,10 +434,8 @@ void launch_patch_offset_one(const DevLayout &d, const PatchArrays &pa, const Of
 }
 
 void launch_patch_offset(int V, const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
-                         int64_t count, double *part, cudaStream_t s) {
+                         int64_t count, double *part, int sms, cudaStream_t s) {
     if (count == 0) return;
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     switch (V) {
         case kOffSame: launch_patch_offset_one<kOffSame>(d, pa, po, first, count, part, sms, s); break;
         case kOffCoarserSrc: launch_patch_offset_one<kOffCoarserSrc>(d, pa, po, first, count, part, sms, s); break;
@@ -452,10 +451,9 @@ size_t patch_smem_bytes(int P, int tab_entries) {
 }
 
 cudaError_t configure_patch_kernels(int P, int tab_entries) {
-    const int bytes = int(patch_smem_bytes(P, tab_entries));
-    if (P == 16)
-        return cudaFuncSetAttribute(patch_interaction_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    return cudaFuncSetAttribute(patch_interaction_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    const size_t bytes = patch_smem_bytes(P, tab_entries);
+    if (P == 16) return opt_in_max_smem(patch_interaction_kernel<16>, bytes);
+    return opt_in_max_smem(patch_interaction_kernel<8>, bytes);
 }
 
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,

@@ -75,6 +75,6 @@ struct OffsetPlan {
 cudaError_t configure_patch_offset();
 // pair class V writes po.n_split slots of [2][count] partial sums at `part` and uses queue counter 1 + V
 void launch_patch_offset(int V, const DevLayout &d, const PatchArrays &pa, const OffsetPlan &po, int64_t first,
-                         int64_t count, double *part, cudaStream_t s);
+                         int64_t count, double *part, int sms, cudaStream_t s);
 
 }  // namespace sg

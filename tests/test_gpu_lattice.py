@@ -1,7 +1,5 @@
 """GPU parity of the lattice-offset reuse path (SG_MODE_LATTICE) against the CPU oracle, at the
 same north_star tolerances as the direct kernel, on all five BASELINE.json configs, plus its edge cases."""
-import os
-
 import numpy as np
 import pytest
 
@@ -56,16 +54,14 @@ def test_small_configs_all_targets(torch_cuda, cfg):
     check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
 
 
-@pytest.mark.parametrize("cfg,seed", [(3, 2003), (4, 2004), (5, 2007)])
-def test_large_configs_sampled_targets(torch_cuda, cfg, seed):
-    """cfg 3: four levels (pairs up to three levels apart: table path and in-kernel direct path); cfg 4: three
-    levels, blocked same-level kernel + cross-level kernel; cfg 5: one level, blocked kernel only."""
-    lay, sigma = make_config(cfg)
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_large_configs_sampled_targets(torch_cuda, large_oracle, cfg):
+    """cfg 3: four levels (pairs up to three levels apart: table path and in-kernel direct path), all 53,248 targets;
+    cfg 4: three levels, all five blocked pair classes, 4,096 stratified targets; cfg 5: one level, blocked same-level
+    kernel only, 4,096 seeded targets.  The oracle samples are the session's (conftest), shared with the direct mode."""
+    lay, sigma, idx, ox, oy = large_oracle(cfg)
+    assert idx.size == (lay.n_cells if cfg == 3 else 4096)
     gx, gy = gpu_force(torch_cuda, lay, sigma)
-    cores = os.cpu_count() or 1
-    n = int(min(4096, max(256, 1.0e8 * min(cores, 64) / lay.n_cells / 4)))
-    idx = sample_targets(lay, n, seed)
-    ox, oy = oracle_force(lay, sigma, idx)
     check(gx[idx], gy[idx], ox, oy)
     assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
 

@@ -1,8 +1,6 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Tolerances are BASELINE.json north_star's: max|dF|/max|F| <= 1e-11 and relative
 L2 <= 1e-12 over both components, FP64 (the oracle side is long double)."""
-import os
-
 import numpy as np
 import pytest
 
@@ -69,22 +67,16 @@ def test_small_configs_all_targets(torch_cuda, cfg):
     check(gx, gy, *oracle_force(lay, sigma))
 
 
-def _n_samples(n_cells):
-    """Oracle budget: about 60 core-seconds of long-double work spread over the host cores."""
-    cores = os.cpu_count() or 1
-    return int(min(4096, max(256, 1.0e8 * min(cores, 64) / n_cells / 4)))
-
-
-@pytest.mark.parametrize("cfg,seed", [(3, 1003), (4, 1004), (5, 1007)])
-def test_large_configs_sampled_targets(torch_cuda, cfg, seed):
-    """Full-size run in the launch configuration bench.py times; oracle on seeded sampled targets
-    (stratified by level), each computed one by one from all N leaves."""
-    lay, sigma = make_config(cfg)
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_large_configs_sampled_targets(torch_cuda, large_oracle, cfg):
+    """Full-size run in the launch configuration bench.py times; oracle coverage as the configs state it (conftest:
+    cfg 3 all 53,248 targets, cfg 4 4,096 stratified by level, cfg 5 4,096 seeded), every oracle value computed one
+    by one from all N leaves in long double."""
+    lay, sigma, idx, ox, oy = large_oracle(cfg)
     exp = expected_counts(cfg)
     assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"]
+    assert idx.size == (lay.n_cells if cfg == 3 else 4096)
     gx, gy = gpu_force(torch_cuda, lay, sigma)
-    idx = sample_targets(lay, _n_samples(lay.n_cells), seed)
-    ox, oy = oracle_force(lay, sigma, idx)
     check(gx[idx], gy[idx], ox, oy)
     # properties that hold at any size: finite everywhere; Newton's third law on the uniform grid
     assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
@@ -220,3 +212,67 @@ def test_state_errors(torch_cuda):
         assert e.value.code == binding.SG_ERR_STATE
         with pytest.raises(SgError):
             d.set_density(torch_cuda.zeros(7, dtype=torch_cuda.float64, device="cuda"))
+
+
+def test_two_live_contexts_of_different_extent(torch_cuda):
+    """Two contexts alive at once, the larger lattice (bigger log table, more dynamic shared memory) created FIRST and
+    the small one after it: the opt-in shared-memory size of a kernel is a per-function, process-wide setting and must
+    not shrink with the last context created.  sg_force calls interleaved, all three modes of use."""
+    from paper_2001_02765_b200 import SgDisk
+    big = nested_layout(4, 64, 8.0, 16)                 # extent 2048 lattice units
+    xb, yb, _ = cell_centres(big)
+    sig_b = kuzmin_sigma(xb, yb, a=0.3)
+    small = uniform_layout(32, -1.0, -1.0, 1 / 16, 16)  # extent 64
+    xs, ys, _ = cell_centres(small)
+    sig_s = kuzmin_sigma(xs, ys)
+    ref_b = oracle_force(big, sig_b)
+    ref_s = oracle_force(small, sig_s)
+    with SgDisk.from_layout(big, device=0) as db:
+        tb = torch_cuda.as_tensor(sig_b).cuda()
+        db.set_density(tb)
+        with SgDisk.from_layout(small, device=0) as ds:
+            ts = torch_cuda.as_tensor(sig_s).cuda()
+            ds.set_density(ts)
+            for mode in ("direct", "lattice", "direct"):
+                ds.set_interaction_mode(mode)
+                db.set_interaction_mode(mode)
+                fs = ds.force()
+                fb = db.force()
+                torch_cuda.cuda.synchronize()
+                check(fb[0].cpu().numpy(), fb[1].cpu().numpy(), *ref_b)
+                check(fs[0].cpu().numpy(), fs[1].cpu().numpy(), *ref_s)
+            # slope path of both (zero slopes: same forces), again large after small
+            zs, zb = torch_cuda.zeros_like(ts), torch_cuda.zeros_like(tb)
+            ds.set_density_linear(ts, zs, zs)
+            db.set_density_linear(tb, zb, zb)
+            fs = ds.force()
+            fb = db.force()
+            torch_cuda.cuda.synchronize()
+            check(fb[0].cpu().numpy(), fb[1].cpu().numpy(), *ref_b)
+            check(fs[0].cpu().numpy(), fs[1].cpu().numpy(), *ref_s)
+
+
+def test_current_device_and_reused_context_with_poisoned_partials(torch_cuda):
+    """One context, many evaluations with changing target ranges and modes: the partial-sum buffer is NaN-filled before
+    every sg_force (SG_POISON_PARTIALS, conftest), so a slot no kernel writes cannot hide behind the previous call's
+    value.  The library leaves the caller's current device as it was."""
+    from paper_2001_02765_b200 import SgDisk
+    lay = nested_layout(5, 64, 8.0, 16)                 # five levels: blocked classes + far pairs (generic kernel)
+    x, y, _ = cell_centres(lay)
+    sigma = kuzmin_sigma(x, y, a=0.3)
+    n = lay.n_cells
+    dev_before = torch_cuda.cuda.current_device()
+    with SgDisk.from_layout(lay, device=0) as d:
+        d.set_density(torch_cuda.as_tensor(sigma).cuda())
+        d.set_interaction_mode("direct")
+        fx, fy = [t.cpu().numpy() for t in d.force()]
+        s = max(np.abs(fx).max(), np.abs(fy).max())
+        for mode in ("lattice", "direct", "lattice"):
+            d.set_interaction_mode(mode)
+            for first, count in ((0, n), (0, 256), (n - 300, 300), (1000, n // 2), (0, n)):
+                d.set_target_range(first, count)
+                gx, gy = [t.cpu().numpy() for t in d.force()]
+                assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy)), (mode, first, count)
+                assert np.abs(gx - fx[first:first + count]).max() <= 1e-12 * s
+                assert np.abs(gy - fy[first:first + count]).max() <= 1e-12 * s
+    assert torch_cuda.cuda.current_device() == dev_before

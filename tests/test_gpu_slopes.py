@@ -106,16 +106,41 @@ def test_random_slopes_conditioning(torch_cuda):
     assert emax <= 1e-9 and l2 <= 1e-9, (emax, l2)
 
 
-@pytest.mark.parametrize("Nk", [128, 256, 512, 1024, 2048])
+_d2_uniform_cache = {}
+
+
+def d2_uniform_gpu(torch, Nk):
+    """The paper's D2 test on the uniform Nk x Nk grid with exact Taylor slopes (R10), slope kernel; the
+    Nk = 2048 run (4.2 M cells, 1.8e13 pairs, ~40 s) is shared by the Table 1 row and the oracle parity check."""
+    if Nk not in _d2_uniform_cache:
+        lay = uniform_layout(Nk, -1.0, -1.0, 2 / Nk, 16)
+        x, y, h = cell_centres(lay)
+        sig = d2_sigma(x, y, 0.5)
+        dx, dy = d2_slopes(x, y, 0.5)
+        Fx, Fy = gpu_force_linear(torch, lay, sig, dx, dy)
+        _d2_uniform_cache.clear()                              # keep one grid at a time (2048^2: 5 x 34 MB)
+        _d2_uniform_cache[Nk] = (lay, x, y, h, sig, dx, dy, Fx, Fy)
+    return _d2_uniform_cache[Nk]
+
+
+def test_slope_kernel_vs_oracle_at_2048_squared(torch_cuda):
+    """The slope kernel against the oracle's first-order sum on 256 seeded targets of the 2048^2 D2 grid (PAPER.md:153,
+    the largest grid of Table 1): excludes GPU drift at 4.2 M cells as the source of the 1.4 % by which the L1/L2
+    columns of that row differ from print (test_paper_table1_D2_uniform_on_gpu below)."""
+    lay, x, y, h, sig, dx, dy, Fx, Fy = d2_uniform_gpu(torch_cuda, 2048)
+    idx = np.sort(np.random.default_rng(2048).choice(lay.n_cells, size=256, replace=False))
+    r = cell_rects(lay)
+    ox, oy, _ = oracle.force(r, sig, r["kxc"][idx], r["kyc"][idx], lay.unit, dx=dx, dy=dy)
+    emax, l2 = errors(Fx[idx], Fy[idx], ox, oy)
+    assert emax <= 1e-11 and l2 <= 1e-12, (emax, l2)
+
+
+@pytest.mark.parametrize("Nk", [2048, 128, 256, 512, 1024])
 def test_paper_table1_D2_uniform_on_gpu(torch_cuda, golden, Nk):
     """PAPER.md:147-153 Table 1, all six columns, from the GPU force (the oracle only reaches Nk = 256 in the CPU
     suite's time budget; Nk = 1024 is 1.1e12 pairs)."""
     row = [r for r in golden("paper_table1_D2_uniform.txt") if int(r[0]) == Nk][0]
-    lay = uniform_layout(Nk, -1.0, -1.0, 2 / Nk, 16)
-    x, y, h = cell_centres(lay)
-    sig = d2_sigma(x, y, 0.5)
-    dx, dy = d2_slopes(x, y, 0.5)
-    Fx, Fy = gpu_force_linear(torch_cuda, lay, sig, dx, dy)
+    lay, x, y, h, sig, dx, dy, Fx, Fy = d2_uniform_gpu(torch_cuda, Nk)
     ax, ay = F_D2_xy(x, y, 0.5)
     R = np.hypot(x, y)
     eR = (Fx * x + Fy * y) / R - (ax * x + ay * y) / R
@@ -124,8 +149,9 @@ def test_paper_table1_D2_uniform_on_gpu(torch_cuda, golden, Nk):
     for g, p in zip(got, row[1:]):
         if Nk == 2048:
             # 4.2 M cells, 1.8e13 pairs: the L-infinity columns agree to the printed digits, the 1- and 2-norms
-            # to 1.4 % (3.60e-6 vs the printed 3.55e-6); the paper's own evaluation is the likelier source (its
-            # primitive -ln(v+r) cancels, R4), so this row is held to 2 %
+            # to 1.4 % (3.60e-6 vs the printed 3.55e-6).  The GPU sum itself agrees with the long-double oracle to
+            # 1e-11 at this size (test_slope_kernel_vs_oracle_at_2048_squared), so the difference is the paper's:
+            # its primitive -ln(v+r) cancels (R4).  This row is held to 2 %.
             assert abs(g - float(p)) <= 0.02 * float(p), (got, row)
         else:
             assert _agree_3_digits(g, p), (got, row)
