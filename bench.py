@@ -9,6 +9,9 @@ independent; :265: "12 cards"), every rank sums over all sources, no data-path c
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
 
+With --gpus N > 1 and no torchrun environment the script re-executes itself under `python -m torch.distributed.run
+--standalone --nproc-per-node N` (one rank per GPU); under torchrun it uses the ranks it is given.
+
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -31,6 +34,7 @@ UNIT = "pairs/s"
 # (SM count and max SM clock from /opt/skills/guides/B200_PROFILING.md; 64 lanes/SM = 4 sub-partitions x 16,
 # consistent with the DFMA micro-benchmark measured live below).  DESIGN.md "Roofline".
 FP64_LANES_PER_SM = 64
+DIRECT_LEG_STEPS = 3          # timed steps of the direct-kernel leg (after 3 warm-ups; SURVEY.md 8(d) protocol)
 
 
 class ClockSampler(threading.Thread):
@@ -82,6 +86,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config list (all five configs)")
     ap.add_argument("--mode", default="auto", choices=["auto", "direct", "lattice"],
                     help="S3 algorithm: direct pair sum, lattice-offset reuse, or auto (lattice when the layout allows)")
     ap.add_argument("--slopes", action="store_true",
@@ -89,50 +94,86 @@ def parse_args():
     return ap.parse_args()
 
 
+KERNEL_SOURCE = {"interaction_kernel": "sg_kernels.cu", "interaction_lin_kernel": "sg_kernels_lin.cu",
+                 "patch_offset_kernel": "sg_kernels_patch.cu", "lattice_corr_kernel": "sg_kernels_lattice.cu"}
+
+
+def kernel_source_sha256(kernel: str):
+    """sha256 of the .cu file that holds `kernel` (the captured traffic figure is tied to it)."""
+    import hashlib
+    for name, fn in KERNEL_SOURCE.items():
+        if kernel.startswith(name):
+            path = os.path.join(ROOT, "paper_2001_02765_b200", "csrc", fn)
+            if os.path.exists(path):
+                return hashlib.sha256(open(path, "rb").read()).hexdigest()
+    return None
+
+
 def measured_traffic(workload: str, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu capture of this
-    workload (profiles/traffic.csv), or None if no capture exists for it."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch, capture id) of `kernel` from the committed ncu
+    capture of this workload (profiles/traffic.csv), or (None, why): ncu cannot run inside the bench, so the figure
+    is a recorded one, and it is dropped when the kernel's source file has changed since the capture."""
     import csv
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(path):
         with open(path) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == workload and kernel.startswith(row["kernel"]):
-                    return int(row["dram_bytes_per_launch"])
-    return None
+                    if row.get("source_sha256") and row["source_sha256"] != kernel_source_sha256(kernel):
+                        return None, f"stale: kernel source changed since capture {row.get('capture')}"
+                    return int(row["dram_bytes_per_launch"]), row.get("capture")
+    return None, "no ncu capture of this kernel on this workload"
 
 
-def amr_side_measurement(torch, device, flush):
-    """BASELINE.json config 4 (three-level AMR, 448,768 leaves) through the same calls, lattice mode: 3 steps of
-    sg_set_density + sg_force between CUDA events after 2 warm-up steps, L2 flushed between steps.  Reported next to
-    the headline (uniform) workload because AMR layouts are what the method is for."""
+def per_config_measurement(torch, device, flush, cfg, nominal_tflops, steps=5, warmup=3):
+    """One BASELINE.json config through the same calls as the headline: `steps` steps of sg_set_density + sg_force
+    between CUDA events after `warmup` warm-up steps, L2 flushed between steps; lattice mode where the layout allows
+    (P = 8 or 16), else the direct kernel.  Roofline fraction on algorithmic units (count x N_v pairs)."""
     from paper_2001_02765_b200 import SgDisk
     from workloads import make_config
-    lay4, sigma4 = make_config(4)
-    with SgDisk.from_layout(lay4, device=device) as d4:
-        d4.set_interaction_mode("lattice")
-        s4 = torch.as_tensor(sigma4).to(torch.device("cuda", device))
-        Fx = torch.empty(lay4.n_cells, dtype=torch.float64, device=s4.device)
+    lay, sigma = make_config(cfg)
+    t0 = time.perf_counter()
+    d = SgDisk.from_layout(lay, device=device)
+    create_ms = (time.perf_counter() - t0) * 1e3
+    try:
+        mode = "lattice" if lay.P in (8, 16) else "direct"
+        t0 = time.perf_counter()
+        d.set_interaction_mode(mode)
+        mode_ms = (time.perf_counter() - t0) * 1e3
+        s = torch.as_tensor(sigma).to(torch.device("cuda", device))
+        Fx = torch.empty(lay.n_cells, dtype=torch.float64, device=s.device)
         Fy = torch.empty_like(Fx)
 
         def step():
             flush.zero_()
-            d4.set_density(s4)
-            d4.force(Fx, Fy)
-        for _ in range(2):
+            d.set_density(s)
+            d.force(Fx, Fy)
+        for _ in range(warmup):
             step()
+        mdl = d.kernel_model()
+        d.set_kernel_timing(True)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record()
-        for _ in range(3):
+        for _ in range(steps):
             step()
         e1.record()
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / 3
-        sd, fl = d4.launch_counts()
-    return {"workload": workload_name(4), "n_cells": lay4.n_cells, "value": float(lay4.n_cells) ** 2 / (ms * 1e-3),
-            "unit": UNIT, "ms_per_step": ms, "steps": 3, "warmup": 2, "gpu_launches_per_step": sd + fl,
-            "interaction_mode": "lattice-offset reuse (SG_MODE_LATTICE): pair classes up to two levels apart"}
+        ms = e0.elapsed_time(e1) / steps
+        kms = d.kernel_times_ms()
+        k = sum(kms) / max(1, len(kms))
+        sd, fl = d.launch_counts()
+    finally:
+        d.close()
+    achieved = mdl["pair_evaluations"] * mdl["flops_per_pair"] / (k * 1e-3) / 1e12
+    return {"config": cfg, "workload": workload_name(cfg), "n_cells": lay.n_cells, "n_levels": lay.n_levels,
+            "patch_cells": lay.P, "interaction_mode": mode, "value": float(lay.n_cells) ** 2 / (ms * 1e-3),
+            "unit": UNIT, "ms_per_step": ms, "interaction_ms": k, "steps": steps, "warmup": warmup,
+            "gpu_launches_per_step": sd + fl, "create_ms": create_ms, "set_mode_ms": mode_ms,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
+                         "frac": achieved / nominal_tflops, "flops_per_pair": mdl["flops_per_pair"],
+                         "pair_evaluations_per_launch": mdl["pair_evaluations"],
+                         "executed_over_algorithmic": mdl["executed_evaluations"] / max(1.0, mdl["pair_evaluations"])}}
 
 
 def workload_name(cfg: int) -> str:
@@ -206,6 +247,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2001_02765_b200 import SgDisk, measure_fp64_peak, shard_range
+    from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
     from workloads import make_config, expected_counts
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -227,9 +269,18 @@ def run_ours(args):
     exp = expected_counts(args.config)
     assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"], "frozen layout changed"
     N = lay.n_cells
-    first, count = shard_range(N, rank, world)
+    lattice = (not args.slopes) and args.mode != "direct" and lay.P in (8, 16)
+    if args.mode == "lattice" and not lattice:
+        raise SystemExit("--mode lattice needs the zeroth-order path and 8x8 or 16x16 patches")
+    if lattice:
+        # lattice mode works on whole patches and a target's cost depends on its level: split by estimated cost
+        first, count = shard_range_by_cost(lattice_patch_costs(lay.patches[:, 0]), lay.P * lay.P, rank, world)
+    else:
+        first, count = shard_range(N, rank, world)
 
+    t_create = time.perf_counter()
     d = SgDisk.from_layout(lay, device=local)
+    create_ms = (time.perf_counter() - t_create) * 1e3
     d.set_target_range(first, count)
     info = d.layout_info()
 
@@ -296,9 +347,6 @@ def run_ours(args):
         d.set_kernel_timing(False)
         return total, kms, clk, mdl
 
-    lattice = (not args.slopes) and args.mode != "direct" and lay.P in (8, 16)
-    if args.mode == "lattice" and not lattice:
-        raise SystemExit("--mode lattice needs the zeroth-order path and 8x8 or 16x16 patches")
     d.set_interaction_mode("lattice" if lattice else "direct")
     sd_launches, f_launches = d.launch_counts()
     ms_total, k_ms, clocks, model = timed_resident(args.steps, max(3, args.warmup))
@@ -306,7 +354,7 @@ def run_ours(args):
     if lattice and world == 1:
         # the north_star kernel (every pair: sqrt + 2 ln) on the same workload, same run, for its roofline line
         d.set_interaction_mode("direct")
-        direct_run = timed_resident(2, 1)
+        direct_run = timed_resident(DIRECT_LEG_STEPS, 3)
         d.set_interaction_mode("lattice")
         step_resident()
 
@@ -333,12 +381,19 @@ def run_ours(args):
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         nominal_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         def roofline_of(mdl, kms, step_ms, kernel, traffic):
-            evals = mdl["pair_evaluations"]                   # algorithmic units one launch processes
+            # achieved: ALGORITHMIC units (count x N_v deduplicated (target, vertex) pairs) x flops
+            # per unit / kernel time.  fp64_pipe_util: the hardware number, from the pairs the kernels EXECUTE
+            # (per-patch vertices in lattice mode, padding slots in direct mode), i.e. what ncu's
+            # sm__pipe_fp64_cycles_active sees (tables and far pairs excluded).
+            evals = mdl["pair_evaluations"]
+            executed = mdl["executed_evaluations"]
             achieved = evals * mdl["flops_per_pair"] / (kms * 1e-3) / 1e12
-            winstr = evals * mdl["fp64_instr_per_pair"] / 32.0 / (kms * 1e-3)      # warp instructions / s
+            winstr = executed * mdl["fp64_instr_per_pair"] / 32.0 / (kms * 1e-3)      # warp instructions / s
+            traffic_bytes, traffic_note = traffic if traffic is not None else (None, "not looked up (multi-GPU run)")
             return {
                 "bound": "alu", "achieved": achieved, "peak": nominal_tflops, "unit": "TFLOP/s",
-                "frac": achieved / nominal_tflops, "traffic": traffic, "kernel": kernel,
+                "frac": achieved / nominal_tflops, "traffic": traffic_bytes, "traffic_capture": traffic_note,
+                "kernel": kernel, "executed_over_algorithmic": executed / max(1.0, evals),
                 "kernel_ms": kms, "kernel_share_of_step": kms / step_ms,
                 "peak_kind": f"nominal {sm_count} SM x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz",
                 "peak_measured_dfma_tflops": peak_tflops, "frac_of_measured_dfma": achieved / peak_tflops,
@@ -351,7 +406,8 @@ def run_ours(args):
         direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
         direct_traffic = measured_traffic(workload_name(args.config), direct_name) if world == 1 else None
         if args.slopes:
-            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>", None)
+            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>",
+                                   measured_traffic(workload_name(args.config), "interaction_lin_kernel<4>") if world == 1 else None)
         elif lattice:
             lattice_name = "patch_offset_kernel<0> (same-level pairs; <1>..<4> for pairs one and two levels apart)"
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, lattice_name,
@@ -366,7 +422,8 @@ def run_ours(args):
                        "pairs_per_evaluation": pairs,
                        "order": "sigma0 + slope terms (Eq. 6)" if args.slopes else "sigma0 (north_star hot path)",
                        "interaction_mode": "lattice-offset reuse (SG_MODE_LATTICE)" if lattice else "direct",
-                       "parallelism": f"targets sharded over {world} GPU(s)",
+                       "parallelism": f"targets sharded over {world} GPU(s)" + (" by estimated cost, whole patches" if lattice else " by count"),
+                       "create_ms": create_ms,
                        "l2": "256 MiB memset between steps (inside the timed region)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N * len(fields), "d2h_bytes_per_step": 16 * count,
                     "ms_per_step": e2e_ms / args.steps},
@@ -378,11 +435,27 @@ def run_ours(args):
             d_k = sum(d_kms) / max(1, len(d_kms))
             line["direct_kernel"] = {
                 "what": "same workload, same run, SG_MODE_DIRECT: every (target, vertex) pair = 1 sqrt + 2 ln "
-                        "(the north_star interaction kernel); 2 timed steps after 1 warm-up",
-                "value": pairs * 2 / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / 2,
-                "roofline": roofline_of(d_model, d_k, d_total / 2, direct_name, direct_traffic)}
-        if world == 1 and args.config == 5 and not args.slopes and lattice:
-            line["amr_workload"] = amr_side_measurement(torch, local, flush)
+                        f"(the north_star interaction kernel); {DIRECT_LEG_STEPS} timed steps after 3 warm-ups",
+                "value": pairs * DIRECT_LEG_STEPS / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / DIRECT_LEG_STEPS,
+                "steps": DIRECT_LEG_STEPS, "warmup": 3,
+                "roofline": roofline_of(d_model, d_k, d_total / DIRECT_LEG_STEPS, direct_name, direct_traffic)}
+        if world == 1 and not args.slopes and not args.no_per_config:
+            # north_star: "report throughput on synthetic disks shaped like the paper's workloads": all five configs,
+            # same calls, same run (the headline workload's own entry repeats the numbers above)
+            line["per_config"] = []
+            for cfg in (1, 2, 3, 4, 5):
+                if cfg == args.config:
+                    line["per_config"].append({
+                        "config": cfg, "workload": workload_name(cfg), "n_cells": N, "n_levels": lay.n_levels,
+                        "patch_cells": lay.P, "interaction_mode": "lattice" if lattice else "direct", "value": value,
+                        "unit": UNIT, "ms_per_step": ms_total / args.steps, "interaction_ms": k_ms_avg,
+                        "steps": args.steps, "warmup": max(3, args.warmup),
+                        "gpu_launches_per_step": sd_launches + f_launches, "create_ms": create_ms,
+                        "roofline": {k: roofline[k] for k in ("bound", "achieved", "peak", "unit", "frac",
+                                                               "flops_per_pair", "pair_evaluations_per_launch",
+                                                               "executed_over_algorithmic")}})
+                else:
+                    line["per_config"].append(per_config_measurement(torch, local, flush, cfg, nominal_tflops))
         if not args.no_cpu_baseline and world == 1:
             rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds)
             line["cpu_baseline"] = {
@@ -395,11 +468,37 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def spawn_command(args, argv):
+    """`python bench.py --gpus N` without a torchrun environment starts the N ranks itself: the command that re-runs
+    this script under torch.distributed.run (one process per GPU, rendezvous on 127.0.0.1), or None when no spawn
+    is needed (N = 1, the reference arm, or already inside a torchrun launch)."""
+    if args.impl != "ours" or args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return None
+    return [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1",
+            f"--nproc-per-node={args.gpus}", "--local-addr", "127.0.0.1", os.path.abspath(__file__), *argv]
+
+
 def main():
     args = parse_args()
+    cmd = spawn_command(args, sys.argv[1:])
+    if cmd is not None:
+        env = dict(os.environ)
+        # NCCL's own log (one "Init COMPLETE" line per rank) goes to stderr; stdout stays the one JSON line
+        env.setdefault("NCCL_DEBUG", "INFO")
+        env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        if os.environ.get("SG_BENCH_PRINT_SPAWN"):             # tests: show the launch instead of running it
+            print(json.dumps({"spawn": cmd}))
+            return
+        sys.stdout.flush()
+        os.execvpe(cmd[0], cmd, env)
     if args.impl == "reference":
         run_reference(args)
     else:
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        if args.gpus != world:
+            raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node "
+                             f"{args.gpus}, or run `python bench.py --gpus {args.gpus}` and let it spawn the ranks")
         run_ours(args)
 
 

@@ -236,3 +236,20 @@ def test_unsupported_patch_size_is_refused(torch_cuda):
         with pytest.raises(SgError) as e:
             d.set_interaction_mode("lattice_blocked")
         assert e.value.code == binding.SG_ERR_ARG
+
+
+def test_cost_based_rank_slices_concatenate_to_the_full_result(torch_cuda):
+    """Multi-GPU sharding of lattice mode (bench.py --gpus N): the cost-balanced, patch-aligned target slices of three
+    "ranks", run one after another on this device, concatenate bit-identically to the unsharded result."""
+    from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
+    lay = nested_layout(5, 64, 8.0, 16)
+    sigma = _noisy_kuzmin(lay, 77)
+    fx, fy = gpu_force(torch_cuda, lay, sigma, "lattice")
+    costs = lattice_patch_costs(lay.patches[:, 0])
+    world = 3
+    px, py = [], []
+    for r in range(world):
+        first, count = shard_range_by_cost(costs, lay.P * lay.P, r, world)
+        gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice", target_range=(first, count))
+        px.append(gx); py.append(gy)
+    assert np.array_equal(np.concatenate(px), fx) and np.array_equal(np.concatenate(py), fy)

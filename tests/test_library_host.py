@@ -178,3 +178,43 @@ def test_lattice_plan_absent_for_other_patch_sizes():
     lay, _ = make_config(2)                                        # P = 8: generic lattice kernel, no offset plan
     with SgDisk.from_layout(lay, device=-1) as d:
         assert not d.lattice_plan_check()["available"]
+
+
+def test_shard_range_by_cost_partitions_whole_patches():
+    from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
+    lay = nested_layout(5, 64, 8.0, 16)                            # five levels: far pairs make coarse targets dearer
+    costs = lattice_patch_costs(lay.patches[:, 0])
+    assert len(costs) == lay.n_patches and len(set(costs)) > 1
+    PP = lay.P * lay.P
+    for world in (1, 2, 3, 8):
+        pieces = [shard_range_by_cost(costs, PP, r, world) for r in range(world)]
+        assert pieces[0][0] == 0 and sum(c for _, c in pieces) == lay.n_cells
+        for (f0, c0), (f1, _) in zip(pieces, pieces[1:]):
+            assert f0 + c0 == f1 and f0 % PP == 0 and c0 % PP == 0
+        share = [sum(costs[f // PP:(f + c) // PP]) for f, c in pieces]
+        assert max(share) - min(share) <= 2 * max(costs)           # balanced to within a patch or two
+
+
+def test_bench_gpus_n_spawns_n_ranks():
+    """`python bench.py --gpus 2` with no torchrun environment re-executes itself under torch.distributed.run with
+    two ranks (the driver's N > 1 command must reach an N-rank run); under torchrun it does not."""
+    import json
+    import subprocess
+    import sys
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env["SG_BENCH_PRINT_SPAWN"] = "1"
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"],
+                         capture_output=True, text=True, env=env, check=True).stdout
+    cmd = json.loads(out.strip().splitlines()[-1])["spawn"]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    assert cmd[-4:] == ["--gpus", "2", "--steps", "1"] and cmd[-5].endswith("bench.py")
+    sys.path.insert(0, ROOT)
+    import bench
+    args = type("A", (), {"impl": "ours", "gpus": 2})()
+    os.environ["WORLD_SIZE"] = "2"
+    try:
+        assert bench.spawn_command(args, []) is None               # already inside a torchrun launch
+    finally:
+        del os.environ["WORLD_SIZE"]
+    assert bench.spawn_command(type("A", (), {"impl": "ours", "gpus": 1})(), []) is None
+    assert bench.spawn_command(type("A", (), {"impl": "reference", "gpus": 4})(), []) is None
