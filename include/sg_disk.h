@@ -144,6 +144,7 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 #define SG_MODE_DIRECT  0
 #define SG_MODE_LATTICE 1
 #define SG_MODE_LATTICE_BLOCKED 2
+#define SG_MODE_LATTICE_INCTA 3
 int sg_set_interaction_mode(sg_ctx *ctx, int mode);
 
 const char *sg_last_error(const sg_ctx *ctx);        /* ctx may be NULL: error of the last failed sg_create */

@@ -217,7 +217,7 @@ class SgDisk:
     def set_interaction_mode(self, mode: str):
         """'direct' (every pair: sqrt + 2 ln), 'lattice' (per-patch-pair offset tables; P = 8 or 16) or
         'lattice_blocked' (the register-blocked offset-table kernels at any size; P = 16)."""
-        self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1, "lattice_blocked": 2}[mode]))
+        self._check(self._lib.sg_set_interaction_mode(self._ctx, {"direct": 0, "lattice": 1, "lattice_blocked": 2, "lattice_incta": 3}[mode]))
 
     def lattice_plan_check(self):
         """Host-side replay of the lattice-mode launch plan (see sg_lattice_plan_check)."""

@@ -10,6 +10,7 @@
 #include "sg_kernels.cuh"
 #include "sg_kernels_lin.cuh"
 #include "sg_kernels_patch.cuh"
+#include "sg_kernels_lattice.cuh"
 #include "sg_layout.h"
 #include "../../include/sg_disk_diag.h"
 
@@ -31,6 +32,10 @@ struct sg_ctx {
     std::vector<PatchGroup> patch_groups;   // the three group lists back to back (offset_group_list)
     int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
     bool use_patch = false;      // sg_set_interaction_mode
+    bool force_incta = false;    // SG_MODE_LATTICE_INCTA: offset tables built inside the CTAs even if the lattices exist
+    LatticeArrays lat;           // precomputed function lattices of the pair classes (sg_kernels_lattice.cu)
+    std::vector<FnLattice> lat_meta;        // host copy, [n_levels * kOffClasses]
+    int64_t lat_entries = 0;                // entries per plane; 0: no plan (P != 16) or over the memory budget
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
@@ -95,7 +100,7 @@ ForcePlan make_plan(const sg_ctx *c, bool linear) {
     ForcePlan p;
     p.first = c->first; p.count = c->count;
     p.smem = linear ? interaction_lin_smem_bytes(c->dev.tab_entries) : interaction_smem_bytes(c->dev.tab_entries);
-    if (p.count == 0) return p;
+    if (p.count == 0 || c->dev.n_tiles == 0) return p;                 // nothing to do / host-only context
     p.T = linear ? lin_targets_per_thread() : (p.count > 16384 ? 4 : 1);
     const int64_t per_block = int64_t(kThreads) * p.T;
     p.n_tblocks = int((p.count + per_block - 1) / per_block);
@@ -207,22 +212,101 @@ OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
 // the pairs >= 3 levels apart; P = 8: generic kernel (tables for pairs <= 1 level apart, direct sum beyond)
 bool use_blocked(const sg_ctx *c, const PatchPlan &) { return c->patch.blocked; }
 
+// Function lattices (sg_kernels_lattice.cuh): extents per (target level, pair class) = the union of the offset boxes
+// of the level's target groups.  Host only; returns the entries per plane (0 if the plan does not exist).
+int64_t plan_fn_lattices(sg_ctx *c) {
+    c->lat_meta.assign(size_t(c->host.n_levels) * kOffClasses, FnLattice{0, 0, 0, 0, 0, 0, 0, 0});
+    if (!c->patch_plan_ok) return 0;
+    const int M_of[kOffClasses] = {32, 48, 47, 80, 77}, TROW_of[kOffClasses] = {33, 49, 49, 81, 79};
+    const int ROWS_of[kOffClasses] = {32, 48, 48, 80, 80};
+    struct Ext { int64_t xlo = INT64_MAX, xhi = INT64_MIN, ylo = INT64_MAX, yhi = INT64_MIN; };
+    std::vector<Ext> ext(c->lat_meta.size());
+    for (const PatchGroup &g : c->patch_groups)
+        for (int v = 0; v < kOffClasses; ++v) {
+            if (g.box[v][1] <= 0 || g.box[v][3] <= 0) continue;
+            const int step = (v == kOffCoarserSrc) ? 2 : (v == kOffCoarserSrc4) ? 4 : 1;
+            Ext &e = ext[size_t(g.level) * kOffClasses + v];
+            e.xlo = std::min<int64_t>(e.xlo, g.box[v][0]);
+            e.xhi = std::max<int64_t>(e.xhi, g.box[v][0] + int64_t(step) * (g.box[v][1] - 1));
+            e.ylo = std::min<int64_t>(e.ylo, g.box[v][2]);
+            e.yhi = std::max<int64_t>(e.yhi, g.box[v][2] + int64_t(step) * (g.box[v][3] - 1));
+        }
+    int64_t total = 0;
+    for (size_t k = 0; k < ext.size(); ++k) {
+        const Ext &e = ext[k];
+        if (e.xlo > e.xhi) continue;
+        const int v = int(k % kOffClasses);
+        const int64_t ncols = 16 * (e.xhi - e.xlo) + TROW_of[v], nrows = 16 * (e.yhi - e.ylo) + std::max(ROWS_of[v], M_of[v]);
+        if (ncols > INT32_MAX / 2 || nrows > INT32_MAX / 2) return 0;
+        FnLattice &m = c->lat_meta[k];
+        m.base = total; m.ncols = int32_t(ncols); m.nrows = int32_t(nrows);
+        m.cmin = int32_t(16 * e.xlo); m.rmin = int32_t(16 * e.ylo); m.present = 1;
+        total += ncols * nrows;
+        total = (total + 7) & ~int64_t(7);                       // every lattice starts on a 128-byte boundary
+    }
+    return total;
+}
+
+// Memory budget of the function lattices (all planes): SG_LATTICE_TABLE_MIB, default 16 GiB.  Over it, lattice mode
+// builds its offset tables inside the CTAs (patch_offset_kernel) and the slope path stays direct.
+int64_t fn_budget_bytes() {
+    const char *e = std::getenv("SG_LATTICE_TABLE_MIB");
+    const int64_t mib = e ? std::atoll(e) : 16384;
+    return std::max<int64_t>(0, mib) << 20;
+}
+
+// Build (or extend to the slope planes) the function lattices.  Host-synchronous; no-op when they exist already.
+int ensure_fn_lattices(sg_ctx *c, int n_planes) {
+    if (c->device < 0 || !c->patch.blocked || c->lat_entries == 0) return SG_OK;
+    if (c->lat.n_planes_built >= n_planes) return SG_OK;
+    if (c->lat_entries * 16 * n_planes > fn_budget_bytes()) return SG_OK;      // stays on the in-CTA tables
+    SG_CUDA(c, cudaDeviceSynchronize());
+    if (c->lat.fn) {
+        cudaFree(c->lat.fn);
+        c->allocs.erase(std::remove(c->allocs.begin(), c->allocs.end(), (void *)c->lat.fn), c->allocs.end());
+        c->dev_bytes -= c->lat_entries * 16 * c->lat.n_planes_built;
+        c->lat.fn = nullptr; c->lat.n_planes_built = 0; c->lat.ready = false;
+    }
+    int rc = dev_alloc(c, &c->lat.fn, c->lat_entries * n_planes);
+    if (rc) return rc;
+    for (FnLattice &m : c->lat_meta) m.plane_stride = c->lat_entries;
+    if (!c->lat.meta) {
+        if ((rc = upload(c, &c->lat.meta, c->lat_meta))) return rc;
+        SG_CUDA(c, configure_lattice_kernels());
+    } else {
+        SG_CUDA(c, cudaMemcpy(c->lat.meta, c->lat_meta.data(), c->lat_meta.size() * sizeof(FnLattice), cudaMemcpyHostToDevice));
+    }
+    c->lat.fn_entries = c->lat_entries;
+    launch_build_fn_lattices(c->lat, c->lat_meta.data(), c->patch_levels.data(), c->host.n_levels, c->dev, 0, n_planes, nullptr);
+    SG_CUDA(c, cudaGetLastError());
+    SG_CUDA(c, cudaDeviceSynchronize());
+    c->lat.n_planes_built = n_planes;
+    c->lat.ready = true;
+    return SG_OK;
+}
+
 // Everything one sg_force launches with the current mode and target range.
 struct StepPlan {
     ForcePlan p;                           // direct / slope kernel, and the finalise kernel (p.n_split partial sums per target)
     PatchPlan pp;                          // generic kernel: everything (P = 8) or the pairs >= 3 levels apart (P = 16)
     OffsetPlan po;                         // blocked kernels: pairs at most two levels apart
     bool by_patch = false, blocked = false, far = true;
+    bool fn = false;                       // blocked kernels read precomputed function lattices (lattice_corr_kernel)
+    int n_planes = 1;                      // 3: slope path in lattice mode
     int64_t partials() const { return int64_t(p.n_split) * 2 * p.count; }
 };
 
 StepPlan make_step_plan(const sg_ctx *c, bool linear) {
     StepPlan sp;
     sp.p = make_plan(c, linear);
-    sp.by_patch = c->use_patch && !linear;
+    // the slope path runs in lattice mode only through the function lattices (three planes)
+    const bool lin_lattice = c->patch.blocked && !c->force_incta && c->lat.n_planes_built >= kFnPlanesLin;
+    sp.by_patch = c->use_patch && (!linear || lin_lattice);
+    sp.n_planes = linear ? kFnPlanesLin : 1;
     if (sp.by_patch) {
         sp.pp = make_patch_plan(c);
         sp.blocked = use_blocked(c, sp.pp);
+        sp.fn = sp.blocked && c->lat.ready && !c->force_incta;
         if (sp.blocked) {
             sp.po = make_offset_plan(c, sp.pp);
             sp.far = c->host.n_levels > 3;                     // pairs >= 3 levels apart exist only then
@@ -379,6 +463,36 @@ int upload_patches(sg_ctx *c) {
     int rc;
     if ((rc = upload(c, &pa.info, c->patch_info))) return rc;
     if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
+    {
+        // owner patch of every vertex: the finest patch that has it on its (P+1)^2 lattice, the lowest index among equals
+        const int P1 = h.P + 1;
+        auto vertex_of = [&](int32_t x, int32_t y) -> int32_t {
+            const auto cx = std::lower_bound(h.colX.begin(), h.colX.end(), x);
+            if (cx == h.colX.end() || *cx != x) return -1;
+            const size_t col = size_t(cx - h.colX.begin());
+            const auto b0 = h.vky.begin() + h.colstart[col], b1 = h.vky.begin() + h.colstart[col + 1];
+            const auto it = std::lower_bound(b0, b1, y);
+            return (it == b1 || *it != y) ? -1 : int32_t(it - h.vky.begin());
+        };
+        std::vector<int32_t> pv(size_t(pa.n_patches) * P1 * P1, -1), owner(size_t(h.Nv), -1);
+        for (int p = 0; p < pa.n_patches; ++p) {
+            const PatchInfo &q = c->patch_info[size_t(p)];
+            for (int j = 0; j < P1; ++j)
+                for (int i = 0; i < P1; ++i) {
+                    const int32_t v = vertex_of(q.X0 + i * q.cw, q.Y0 + j * q.cw);
+                    pv[(size_t(p) * P1 + j) * P1 + i] = v;
+                    if (v < 0) continue;                           // cannot happen: every patch vertex is a cell corner
+                    int32_t &o = owner[size_t(v)];
+                    if (o < 0 || c->patch_info[size_t(o)].level < q.level) o = p;
+                }
+        }
+        for (int p = 0; p < pa.n_patches; ++p)
+            for (int e = 0; e < P1 * P1; ++e) {
+                int32_t &v = pv[size_t(p) * P1 * P1 + e];
+                if (v >= 0 && owner[size_t(v)] != p) v = -1;
+            }
+        if ((rc = upload(c, &pa.pvmap, pv))) return rc;
+    }
     SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
     if (pa.P == 16) {
         const bool ok = c->patch_plan_ok;
@@ -389,6 +503,19 @@ int upload_patches(sg_ctx *c) {
             if ((rc = upload(c, &pa.levels, lev)) || (rc = upload(c, &pa.groups, groups)) || (rc = upload(c, &pa.pmap, pmap)))
                 return rc;
             if ((rc = dev_alloc(c, &pa.wQ, int64_t(pa.n_patches) * kPatchQStride))) return rc;
+            // per level: the patches at least three levels away (patch_far_kernel)
+            std::vector<int32_t> far_list, far_meta(size_t(2 * h.n_levels), 0);
+            for (int L = 0; L < h.n_levels; ++L) {
+                far_meta[size_t(2 * L)] = int32_t(far_list.size());
+                for (int M2 = 0; M2 < h.n_levels; ++M2) {
+                    if (std::abs(M2 - L) < 3) continue;
+                    for (size_t q = 0; q < h.patches.size(); ++q)
+                        if (h.patches[q].level == M2) far_list.push_back(int32_t(q));
+                }
+                far_meta[size_t(2 * L + 1)] = int32_t(far_list.size()) - far_meta[size_t(2 * L)];
+            }
+            if ((rc = upload(c, &pa.far_list, far_list)) || (rc = upload(c, &pa.far_meta, far_meta))) return rc;
+            SG_CUDA(c, configure_patch_far(c->dev.tab_entries));
             pa.n_groups = int(groups.size());
             SG_CUDA(c, configure_patch_offset());
             pa.blocked = true;
@@ -467,6 +594,7 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
         c->dev.G = G;
         c->first = 0; c->count = c->host.N;
         c->patch_plan_ok = build_patch_plan(c);
+        c->lat_entries = plan_fn_lattices(c);
         if (device >= 0) {
             DeviceGuard guard(device);
             cudaError_t e = guard.err;
@@ -538,7 +666,7 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     SG_CUDA(c, guard.err);
     launch_vertex_weights(c->dev, sigma_dev, s);
     launch_line_tables(c->dev, s);
-    if (c->patch.enabled) launch_patch_weights(c->patch, sigma_dev, s);
+    if (c->patch.enabled) launch_patch_weights(c->patch, c->dev.w, s);
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = false;
@@ -568,10 +696,15 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
         if ((rc = dev_alloc(c, &l.TBx3, int64_t(d.ntY) * d.nX * 3))) return rc;
         if ((rc = dev_alloc(c, &l.TBy3, int64_t(d.ntX) * d.nY * 3))) return rc;
         SG_CUDA(c, configure_lin_kernels(d.tab_entries));
+        if (c->patch.blocked && (rc = dev_alloc(c, &c->lat.wS, int64_t(kFnPlanesLin) * c->patch.n_patches * kPatchQStride)))
+            return rc;
         l.allocated = true;
+        // lattice mode is on already: add the slope planes to the function lattices (host-synchronous, first call only)
+        if (c->use_patch && !c->force_incta && (rc = ensure_fn_lattices(c, kFnPlanesLin))) return rc;
         if ((rc = reserve_partials(c))) return rc;
     }
     launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
+    if (c->lat.wS) launch_patch_weights_lin(c->patch, l.wl, c->lat.wS, s);
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = true;
@@ -597,7 +730,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
         SG_CUDA(c, cudaMemsetAsync(c->dev.part, 0xFF, size_t(sp.partials()) * sizeof(double), s));
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
-    if (c->linear) launch_interaction_lin(c->dev, c->lin, p, s);
+    if (c->linear && !sp.by_patch) launch_interaction_lin(c->dev, c->lin, p, s);
     else if (sp.by_patch) {
         // every launch writes its own n_split slots of [2][count] partial sums and has its own work queue, so the
         // launches are independent: the first runs on the caller's stream, the others on side streams that wait for
@@ -634,16 +767,24 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
         if (sp.blocked)
             for (int v = 0; v < kOffClasses; ++v)
                 if (po.variant[v]) {
-                    launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, c->sm_count, on_stream(n_launch));
+                    if (sp.fn)
+                        launch_lattice_corr(v, c->dev, c->patch, c->lat, po, sp.n_planes, c->first, c->count, part, c->sm_count,
+                                            on_stream(n_launch));
+                    else
+                        launch_patch_offset(v, c->dev, c->patch, po, c->first, c->count, part, c->sm_count, on_stream(n_launch));
                     ++n_launch;
                     part += int64_t(po.n_split) * 2 * c->count;
                     if (debug_sync && first_err == cudaSuccess) {
                         const cudaError_t e = cudaDeviceSynchronize();
-                        if (e != cudaSuccess) { first_err = e; where = "patch_offset_kernel<" + std::to_string(v) + ">"; }
+                        if (e != cudaSuccess) { first_err = e; where = std::string(sp.fn ? "lattice_corr_kernel<" : "patch_offset_kernel<") + std::to_string(v) + ">"; }
                     }
                 }
-        if (!sp.blocked || sp.far) {
-            launch_patch_interaction(c->dev, c->patch, sp.pp, c->first, c->count, part, sp.blocked ? 3 : 0, on_stream(n_launch));
+        if (sp.blocked && sp.far) {                            // pairs >= 3 levels apart, directly
+            launch_patch_far(c->linear, c->dev, c->patch, c->linear ? c->lat.wS : c->patch.wQ, sp.pp, c->first, c->count, part,
+                             on_stream(n_launch));
+            ++n_launch;
+        } else if (!sp.blocked) {                              // P = 8: everything in the generic kernel
+            launch_patch_interaction(c->dev, c->patch, sp.pp, c->first, c->count, part, 0, on_stream(n_launch));
             ++n_launch;
         }
         note(cudaGetLastError(), "pair-class kernel launch");
@@ -671,20 +812,26 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
 
 int sg_set_interaction_mode(sg_ctx *c, int mode) {
     if (!c) return SG_ERR_ARG;
-    if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE && mode != SG_MODE_LATTICE_BLOCKED) {
+    if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE && mode != SG_MODE_LATTICE_BLOCKED && mode != SG_MODE_LATTICE_INCTA) {
         c->err = "unknown interaction mode"; return SG_ERR_ARG;
     }
     if (mode == SG_MODE_LATTICE && c->host.P != 8 && c->host.P != 16) {
         c->err = "SG_MODE_LATTICE needs patches of 8 x 8 or 16 x 16 cells"; return SG_ERR_ARG;
     }
-    if (mode == SG_MODE_LATTICE_BLOCKED && (c->host.P != 16 || (c->device >= 0 && !c->patch.blocked))) {
-        c->err = "SG_MODE_LATTICE_BLOCKED needs patches of 16 x 16 cells (and per-level patch maps that fit)";
+    if ((mode == SG_MODE_LATTICE_BLOCKED || mode == SG_MODE_LATTICE_INCTA) &&
+        (c->host.P != 16 || (c->device >= 0 && !c->patch.blocked))) {
+        c->err = "SG_MODE_LATTICE_BLOCKED / _INCTA need patches of 16 x 16 cells (and per-level patch maps that fit)";
         return SG_ERR_ARG;
     }
     c->use_patch = mode != SG_MODE_DIRECT;
+    c->force_incta = mode == SG_MODE_LATTICE_INCTA;
     if (c->device < 0) return SG_OK;
     DeviceGuard guard(c->device);
     SG_CUDA(c, guard.err);
+    if (c->use_patch && !c->force_incta) {
+        const int rc = ensure_fn_lattices(c, c->lin.allocated ? kFnPlanesLin : 1);
+        if (rc) return rc;
+    }
     return reserve_partials(c);
 }
 
@@ -760,16 +907,13 @@ int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
 int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     if (!c) return SG_ERR_ARG;
     // vertex weights, running sums and look-ups per direction (+ per-patch weights when the lattice-offset path exists);
-    // with slopes: weights, column tables, row tables
-    if (set_density_launches) *set_density_launches = c->linear ? 3 : 5 + (c->patch.enabled ? 1 : 0);
+    // with slopes: weights, column tables, row tables (+ per-patch slope weights)
+    if (set_density_launches) *set_density_launches = c->linear ? 3 + (c->lat.wS ? 1 : 0) : 5 + (c->patch.enabled ? 1 : 0);
     if (force_launches) {                                         // interaction kernel(s) + finalise
         int n = 1;
-        if (c->use_patch && !c->linear && c->count > 0) {
-            const PatchPlan pp = make_patch_plan(c);
-            if (use_blocked(c, pp)) {
-                const OffsetPlan po = make_offset_plan(c, pp);
-                n = offset_classes(po) + (c->host.n_levels > 3 ? 1 : 0);
-            }
+        if (c->count > 0) {
+            const StepPlan sp = make_step_plan(c, c->linear);
+            if (sp.by_patch && sp.blocked) n = offset_classes(sp.po) + (sp.far ? 1 : 0);
         }
         *force_launches = c->count > 0 ? n + 1 : 0;
     }
@@ -817,7 +961,16 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
     // algorithmic unit: one (target, deduplicated vertex) pair; one launch processes count * N_v
     const double alg = double(c->count) * double(c->host.Nv);
     if (pair_evaluations) *pair_evaluations = alg;
-    if (c->use_patch && !c->linear) {
+    const StepPlan sp = make_step_plan(c, c->linear);
+    if (sp.by_patch && c->linear) {
+        // slope path in lattice mode: three planes, 6 DFMA per pair (sg_kernels_lattice.cu)
+        if (fp64_instr_per_pair) *fp64_instr_per_pair = 6.0;
+        if (flops_per_pair) *flops_per_pair = 12.0;
+        if (executed_evaluations)
+            *executed_evaluations = double(c->count) * double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
+        return SG_OK;
+    }
+    if (sp.by_patch) {
         // lattice-offset path: a pair costs the 2 DFMA of the correlation.  The kernels work on per-patch vertex
         // sets, (P+1)^2 / P^2 more pairs than the deduplicated list: reported separately as executed work, not
         // credited.  Not credited either: the offset tables and the pairs >= 3 levels apart that are summed

@@ -248,7 +248,7 @@ __global__ void finalise_lin_kernel(const double2 *__restrict__ tgt, const int32
                                     unsigned int *__restrict__ queue, const double *__restrict__ lnint,
                                     int lnint_n) {
     const int64_t lt = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (lt == 0) *queue = 0u;
+    if (lt < kQueues) queue[lt] = 0u;                 // every work queue (lattice mode uses one per pair class)
     if (lt >= count) return;
     const int64_t t = first + lt;
     const double2 p = tgt[t];

@@ -21,38 +21,52 @@
 
 #include "sg_device.cuh"
 #include "sg_kernels_patch.cuh"
+#include "sg_patch_device.cuh"
 
 namespace sg {
 
 constexpr int kPatchMaxM = 48;        // table path for |level difference| <= 1: M <= 3P <= 48
 
-// per-patch signed vertex weights: vertex (i,j) of patch p is the NE corner of its cell (i-1,j-1) (+), the NW
-// corner of (i,j-1) (-), the SE corner of (i-1,j) (-) and the SW corner of (i,j) (+)   [[.]] of PAPER.md:92
-// wQ (P = 16 only, may be null): the same weights with rows 18 apart (column 17 zero) so that patch_offset_kernel
-// stages them with aligned 16-byte copies.
-__global__ void patch_weights_kernel(const double *__restrict__ sigma, double *__restrict__ wP, double *__restrict__ wQ,
-                                     int P, int wstride, int n_patches) {
-    const int p = blockIdx.x;
-    const double *s = sigma + int64_t(p) * P * P;
-    for (int e = threadIdx.x; e < wstride; e += blockDim.x) {
-        double w = 0.0;
-        if (e < (P + 1) * (P + 1)) {
-            const int i = e % (P + 1), j = e / (P + 1);
-            if (i >= 1 && j >= 1) w += s[(j - 1) * P + (i - 1)];
-            if (i < P && j >= 1) w -= s[(j - 1) * P + i];
-            if (i >= 1 && j < P) w -= s[j * P + (i - 1)];
-            if (i < P && j < P) w += s[j * P + i];
-            if (wQ) {
-                wQ[int64_t(p) * kPatchQStride + j * (P + 2) + i] = w;
-                if (i == P) wQ[int64_t(p) * kPatchQStride + j * (P + 2) + P + 1] = 0.0;
+// Per-patch vertex weights = the DEDUPLICATED signed vertex weights w_v (vertex_weights_kernel: the sum of +-sigma over
+// all <= 4 cells around v, whichever patch they belong to), each global vertex handed to exactly ONE owner patch
+// (pvmap[p][j][i] = vertex index if patch p owns vertex (i, j) of its (P+1)^2 lattice, else -1; sg_create picks the
+// finest patch that has the vertex, the lowest index among equals).  The sum over patches is then the same sum over
+// vertices as in the direct kernel, and the weights a patch correlates are second differences of sigma (small for a
+// smooth disk) instead of one-sided patch-edge sums that only cancel against the neighbouring patch: an order of
+// magnitude less rounding error, for the slope path in particular.
+// wP: [j][i] rows P+1 apart (generic kernel).  wQ (P = 16 only, may be null): rows 18 apart, column 17 zero, so that the
+// offset-table kernels read aligned 16-byte pairs.  n_planes = 1: plane 0 = w[v];  3 (slope path): planes -W0, a, c
+// from wl[3 v + {0, 1, 2}] (vertex_weights_lin_kernel), wQ layout only.
+__global__ void patch_weights_kernel(const double *__restrict__ w, const int32_t *__restrict__ pvmap,
+                                     double *__restrict__ wP, double *__restrict__ wQ, int P, int wstride,
+                                     int n_planes, int64_t q_plane_stride) {
+    const int p = blockIdx.x, NV = (P + 1) * (P + 1);
+    for (int e = threadIdx.x; e < max(wstride, kPatchQStride); e += blockDim.x) {
+        if (n_planes == 1 && e < wstride) {
+            const int v = e < NV ? pvmap[int64_t(p) * NV + e] : -1;
+            wP[int64_t(p) * wstride + e] = v >= 0 ? w[v] : 0.0;
+        }
+        if (wQ && e < kPatchQStride) {
+            const int i = e % (P + 2), j = e / (P + 2);
+            const int v = i <= P ? pvmap[int64_t(p) * NV + j * (P + 1) + i] : -1;
+            if (n_planes == 1) wQ[int64_t(p) * kPatchQStride + e] = v >= 0 ? w[v] : 0.0;
+            else {
+                const int64_t o = int64_t(p) * kPatchQStride + e;
+                wQ[o] = v >= 0 ? -w[3 * int64_t(v)] : 0.0;
+                wQ[q_plane_stride + o] = v >= 0 ? w[3 * int64_t(v) + 1] : 0.0;
+                wQ[2 * q_plane_stride + o] = v >= 0 ? w[3 * int64_t(v) + 2] : 0.0;
             }
         }
-        wP[int64_t(p) * wstride + e] = w;
     }
 }
 
-void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s) {
-    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, pa.wP, pa.wQ, pa.P, pa.wstride, pa.n_patches);
+void launch_patch_weights(const PatchArrays &pa, const double *w, cudaStream_t s) {
+    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(w, pa.pvmap, pa.wP, pa.wQ, pa.P, pa.wstride, 1, 0);
+}
+
+void launch_patch_weights_lin(const PatchArrays &pa, const double *wl, double *wS, cudaStream_t s) {
+    patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(wl, pa.pvmap, nullptr, wS, pa.P, pa.wstride, 3,
+                                                      int64_t(pa.n_patches) * kPatchQStride);
 }
 
 __device__ __forceinline__ double2 pair_terms(double u, double v, const char *tabb, uint32_t keep) {
@@ -158,6 +172,123 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 }
 
 // ------------------------------------------------------------------------------------------------
+// Patch pairs three or more levels apart, P = 16 (table side >= 137: no reuse left): every (target, vertex) pair
+// directly, 21 FP64-pipe instructions (28 with the slope terms, LIN), column by column as in interaction_kernel
+// (u, u^2 and s(u) once per column, v by exact integer steps).  Work item = (target patch, split of the list of the
+// source patches that are far from the target's level); the lists are per level (far_meta[2 l] = first entry,
+// [2 l + 1] = count), so every item of a level carries the same work.  Weights in the wQ layout (rows 18 apart);
+// LIN: planes -W0, a, c (patch_weights_kernel) and the partial sums hold the main parts of F/G as in
+// interaction_lin_kernel.
+// ------------------------------------------------------------------------------------------------
+template <bool LIN>
+__global__ void __launch_bounds__(256, 2)
+patch_far_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ wq, int64_t w_plane_stride,
+                 const int32_t *__restrict__ far_list, const int32_t *__restrict__ far_meta,
+                 const double *__restrict__ lntab_g, int tab_idx0, int tab_entries, int n_split, int first_patch,
+                 int n_tpatches, int64_t first, int64_t count, double *__restrict__ part,
+                 unsigned int *__restrict__ queue, uint32_t keep) {
+    constexpr int P = 16, NT = P * P, NPL = LIN ? 3 : 1;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *sw = reinterpret_cast<double *>(smem_raw);                    // [NPL][kPatchQStride] weights of B
+    double *stab = sw + NPL * kPatchQStride;                              // log table
+    __shared__ int s_item;
+    const int tid = threadIdx.x, k = tid % P, l = tid / P;
+
+    for (int i = tid; i < tab_entries; i += NT) stab[i] = lntab_g[i];
+    const char *tabb = reinterpret_cast<const char *>(stab) - int64_t(tab_idx0) * 8 - 4;
+
+    const int n_items = n_tpatches * n_split;
+    while (true) {
+        __syncthreads();
+        if (tid == 0) s_item = int(atomicAdd(queue, 1u));
+        __syncthreads();
+        const int item = s_item;
+        if (item >= n_items) break;
+        const int ta = item / n_split, sp = item - ta * n_split;
+        const PatchInfo A = info[first_patch + ta];
+        const int f0 = far_meta[2 * A.level], fc = far_meta[2 * A.level + 1];
+        const int per = (fc + n_split - 1) / n_split;
+        const int b0 = sp * per, b1 = min(fc, b0 + per);
+        const int xt = A.X0 + k * A.cw + A.cw / 2, yt = A.Y0 + l * A.cw + A.cw / 2;     // lattice, exact
+        double ax = 0.0, ay = 0.0;
+        for (int bb = b0; bb < b1; ++bb) {
+            const int b = far_list[f0 + bb];
+            const PatchInfo B = info[b];
+            __syncthreads();                                   // previous source patch is done with sw
+            for (int e = tid; e < NPL * kPatchQStride; e += NT)
+                sw[e] = wq[int64_t(e / kPatchQStride) * w_plane_stride + int64_t(b) * kPatchQStride + e % kPatchQStride];
+            __syncthreads();
+            const double dv = double(B.cw), v0 = double(B.Y0 - yt);
+            for (int i = 0; i <= P; ++i) {
+                const double u = double(B.X0 + i * B.cw - xt), uu = u * u, au = fabs(u);
+                double cy = 0.0, cx2 = 0.0, cy1 = 0.0, v = v0;
+#pragma unroll 4
+                for (int j = 0; j <= P; ++j, v += dv) {
+                    const double w = sw[j * (P + 2) + i];
+                    const double q = fma(v, v, uu);
+                    const double y0 = rsqrt_approx(q);
+                    const double t = q * y0;
+                    const double e = fma(-t, y0, 1.0);
+                    const double pp = fma(0.375, e, 0.5);
+                    const double r = fma(t, pp * e, t);
+                    const double sl1 = flip_sign_by(fast_ln(fabs(v) + r, tabb, keep), v);
+                    const double l2 = fast_ln(au + r, tabb, keep);
+                    if (!LIN) {
+                        ax = fma(w, sl1, ax);
+                        cy = fma(w, l2, cy);
+                    } else {
+                        // w = -W0;  Wt = W0 - u a - v c;  x: -Wt s(v)L1 + a v s(u)L2 - c r;  y: -Wt s(u)L2 + c u s(v)L1 - a r
+                        const double a = sw[kPatchQStride + j * (P + 2) + i], c = sw[2 * kPatchQStride + j * (P + 2) + i];
+                        const double mwt = fma(v, c, fma(u, a, w));           // -Wt
+                        ax = fma(mwt, sl1, ax);
+                        ax = fma(-c, r, ax);
+                        cx2 = fma(a * v, l2, cx2);
+                        cy = fma(mwt, l2, cy);
+                        cy1 = fma(c, sl1, cy1);
+                        ay = fma(-a, r, ay);
+                    }
+                }
+                ay += flip_sign_by(cy, u);
+                if (LIN) {
+                    ax += flip_sign_by(cx2, u);
+                    ay = fma(u, cy1, ay);
+                }
+            }
+        }
+        const int64_t lt = (int64_t(first_patch + ta) * NT + tid) - first;      // local index in the target range
+        if (lt >= 0 && lt < count) {
+            part[(int64_t(sp) * 2 + 0) * count + lt] = ax;
+            part[(int64_t(sp) * 2 + 1) * count + lt] = ay;
+        }
+    }
+}
+
+size_t patch_far_smem_bytes(bool lin, int tab_entries) {
+    return size_t(lin ? 3 : 1) * kPatchQStride * 8 + size_t(tab_entries) * 8;
+}
+
+cudaError_t configure_patch_far(int tab_entries) {
+    cudaError_t e = opt_in_max_smem(patch_far_kernel<false>, patch_far_smem_bytes(false, tab_entries));
+    if (e == cudaSuccess) e = opt_in_max_smem(patch_far_kernel<true>, patch_far_smem_bytes(true, tab_entries));
+    return e;
+}
+
+void launch_patch_far(bool lin, const DevLayout &d, const PatchArrays &pa, const double *wq, const PatchPlan &pp,
+                      int64_t first, int64_t count, double *part, cudaStream_t s) {
+    if (count == 0) return;
+    const int64_t stride = int64_t(pa.n_patches) * kPatchQStride;
+    const size_t smem = patch_far_smem_bytes(lin, d.tab_entries);
+    if (lin)
+        patch_far_kernel<true><<<pp.grid, 256, smem, s>>>(pa.info, wq, stride, pa.far_list, pa.far_meta, d.lntab, d.tab_idx0,
+                                                         d.tab_entries, pp.n_split, pp.first_patch, pp.n_tpatches, first,
+                                                         count, part, d.queue, kLogKeepMask);
+    else
+        patch_far_kernel<false><<<pp.grid, 256, smem, s>>>(pa.info, wq, stride, pa.far_list, pa.far_meta, d.lntab, d.tab_idx0,
+                                                          d.tab_entries, pp.n_split, pp.first_patch, pp.n_tpatches, first,
+                                                          count, part, d.queue, kLogKeepMask);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Patch pairs at most two levels apart, P = 16: register-blocked correlation with ONE OFFSET TABLE PER CTA.
 //
 // The table of a patch pair depends only on the patch offset d = B - A (in units of the finer level's patch size)
@@ -183,50 +314,6 @@ patch_interaction_kernel(const PatchInfo *__restrict__ info, const double *__res
 // number of entries apart so that the 8 lanes of an LDS.128 quarter-warp hit 8 different 16-byte bank groups.
 // Every per-patch sum stays in one accumulator chain (split chains cancel badly).
 // ------------------------------------------------------------------------------------------------
-constexpr int kOffWarps = 8, kBlkR = 8, kBlkWRow = 32, kBlkW = 17 * kBlkWRow;
-
-__device__ __forceinline__ double fast_ln_g(double a, const double *__restrict__ lntab_g, int tab_idx0, uint32_t keep) {
-    const uint32_t hi = uint32_t(__double2hiint(a));
-    const uint32_t hc = (hi & keep) | kLogHalfBin;
-    const double tv = __ldg(lntab_g + (int(hc >> kLogShift) - tab_idx0));
-    const double c = rcp_approx(__hiloint2double(int(hc), 0));
-    const double f = fma(a, c, -1.0);
-    double s = fma(f, -0.25, 1.0 / 3.0);
-    s = fma(f, s, -0.5);
-    s = fma(f, s, 1.0);
-    return fma(f, s, tv);
-}
-
-__device__ __forceinline__ double2 pair_terms_g(double u, double v, const double *__restrict__ lntab_g, int tab_idx0,
-                                                uint32_t keep) {
-    const double q = fma(u, u, v * v);
-    const double y0 = rsqrt_approx(q);
-    const double t = q * y0;
-    const double e = fma(-t, y0, 1.0);
-    const double p = fma(0.375, e, 0.5);
-    const double r = fma(t, p * e, t);
-    return make_double2(flip_sign_by(fast_ln_g(fabs(v) + r, lntab_g, tab_idx0, keep), v),
-                        flip_sign_by(fast_ln_g(fabs(u) + r, lntab_g, tab_idx0, keep), u));
-}
-
-// compile-time description of pair class V (kOffSame, kOffCoarserSrc, kOffFinerSrc, kOffCoarserSrc4, kOffFinerSrc4)
-template <int V>
-struct OffCls {
-    static constexpr int P = 16;
-    static constexpr bool coarser = V == kOffCoarserSrc || V == kOffCoarserSrc4, finer = V == kOffFinerSrc || V == kOffFinerSrc4;
-    static constexpr int F = V == kOffSame ? 1 : (V == kOffCoarserSrc || V == kOffFinerSrc) ? 2 : 4;   // pitch ratio
-    static constexpr int RA = finer ? F : 1, RB = coarser ? F : 1;        // target / source pitch in units of g
-    static constexpr int M = P * RB + (P - 1) * RA + 1, MMIN = (P - 1) * RA;      // table side 32, 48, 47, 80, 77
-    static constexpr int RPC = (M + RA - 1) / RA;                         // stored rows per row class (finer source)
-    static constexpr int ROWS = RA * RPC, TROW = (M | 1) == M ? M + 2 : M + 1;    // odd pitch >= M + 1
-    static constexpr int TBUF = ROWS * TROW;
-    static constexpr bool DB = F < 4;                                     // double-buffered tables (two CTAs per SM)
-    static constexpr int LDIST = coarser ? -(F == 2 ? 1 : 2) : finer ? (F == 2 ? 1 : 2) : 0;   // source level - target level
-    static constexpr bool WG = F == 4;                                    // weights straight from global / L1: the table
-                                                                          // leaves no room for weight buffers at 2 CTAs per SM
-    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16 + (WG ? 0 : size_t(kOffWarps) * kBlkW * 8);
-};
-
 template <int V>
 __global__ void __launch_bounds__(kOffWarps * 32, 2)
 patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,

@@ -49,7 +49,10 @@ struct PatchArrays {
     int n_patches = 0;
     int wstride = 0;                  // doubles per patch in wP: (P+1)^2 rounded up to a multiple of 2
     PatchInfo *info = nullptr;        // [n_patches]
-    double *wP = nullptr;             // [n_patches * wstride] per-patch signed vertex weights, [j][i]
+    double *wP = nullptr;             // [n_patches * wstride] per-patch (owned, deduplicated) vertex weights, [j][i]
+    int32_t *far_list = nullptr;      // P = 16: per level, the patches >= 3 levels away (patch_far_kernel)
+    int32_t *far_meta = nullptr;      // [2 n_levels]: first entry and count of every level's list
+    int32_t *pvmap = nullptr;         // [n_patches * (P+1)^2] global vertex owned by patch vertex (i, j), or -1
 };
 
 struct PatchPlan {
@@ -61,10 +64,16 @@ struct PatchPlan {
 
 size_t patch_smem_bytes(int P, int tab_entries);
 cudaError_t configure_patch_kernels(int P, int tab_entries);
-void launch_patch_weights(const PatchArrays &pa, const double *sigma, cudaStream_t s);
+// w: flat deduplicated vertex weights (DevLayout::w); wl: {W0, a, c} per vertex of the slope path (LinArrays::wl)
+void launch_patch_weights(const PatchArrays &pa, const double *w, cudaStream_t s);
+void launch_patch_weights_lin(const PatchArrays &pa, const double *wl, double *wS, cudaStream_t s);
 // skip_near: patch pairs fewer than skip_near levels apart are skipped (done by patch_offset_kernel); 0 = none
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
                               int64_t count, double *part, int skip_near, cudaStream_t s);
+// P = 16: pairs >= 3 levels apart summed directly; wq: pa.wQ (zeroth order) or the three slope planes (lin)
+cudaError_t configure_patch_far(int tab_entries);
+void launch_patch_far(bool lin, const DevLayout &d, const PatchArrays &pa, const double *wq, const PatchPlan &pp,
+                      int64_t first, int64_t count, double *part, cudaStream_t s);
 // register-blocked kernels with one offset table per CTA (P = 16), patch pairs at most two levels apart
 struct OffsetPlan {
     int n_groups[3] = {0, 0, 0};      // sizes of the three group lists, stored back to back

@@ -104,13 +104,35 @@ def _noisy_kuzmin(lay, seed, a=0.3):
     return kuzmin_sigma(x, y, a=a) * (1 + 0.2 * np.random.default_rng(seed).uniform(-1, 1, lay.n_cells))
 
 
-def test_blocked_kernels_four_nested_levels(torch_cuda):
-    """P = 16, four nested levels, ALL targets vs the oracle with the register-blocked offset-table kernels forced
-    (SG_MODE_LATTICE_BLOCKED): same-level, coarser-source and finer-source classes plus the direct far pairs."""
+@pytest.mark.parametrize("mode", ["lattice_blocked", "lattice_incta"])
+def test_blocked_kernels_four_nested_levels(torch_cuda, mode):
+    """P = 16, four nested levels, ALL targets vs the oracle with the register-blocked kernels: all five pair classes
+    plus the directly summed far pairs.  lattice_blocked: tables streamed from the precomputed function lattices
+    (lattice_corr_kernel); lattice_incta: tables built inside the CTAs (patch_offset_kernel)."""
     lay = nested_layout(4, 64, 8.0, 16)
     sigma = _noisy_kuzmin(lay, 21)
-    gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice_blocked")
+    gx, gy = gpu_force(torch_cuda, lay, sigma, mode)
     check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+
+
+def test_function_lattices_and_in_cta_tables_agree_bitwise(torch_cuda):
+    """The precomputed function lattices hold the values the in-CTA tables compute and the correlation order is the
+    same: both variants give bit-identical forces (cfg 4: all five classes, irregular levels)."""
+    lay, sigma = make_config(4)
+    a = gpu_force(torch_cuda, lay, sigma, "lattice")
+    b = gpu_force(torch_cuda, lay, sigma, "lattice_incta")
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_function_lattice_budget_falls_back_to_in_cta_tables(torch_cuda, monkeypatch):
+    """With a memory budget too small for the function lattices (SG_LATTICE_TABLE_MIB), lattice mode builds its tables
+    inside the CTAs: same result."""
+    lay = nested_layout(3, 64, 4.0, 16)
+    sigma = _noisy_kuzmin(lay, 8)
+    a = gpu_force(torch_cuda, lay, sigma, "lattice")
+    monkeypatch.setenv("SG_LATTICE_TABLE_MIB", "1")
+    b = gpu_force(torch_cuda, lay, sigma, "lattice")
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
 
 
 @pytest.mark.parametrize("seed", [1, 2])
@@ -210,12 +232,13 @@ def test_fuzz_random_hierarchies_lattice_vs_direct(torch_cuda):
             d.set_density(torch_cuda.as_tensor(sigma).cuda())
             d.set_target_range(first, count)
             out = {}
-            for mode in ("direct", "lattice"):
+            for mode in ("direct", "lattice", "lattice_incta"):
                 d.set_interaction_mode(mode)
                 Fx, Fy = d.force()
                 torch_cuda.cuda.synchronize()
                 out[mode] = (Fx.cpu().numpy(), Fy.cpu().numpy())
         (ax, ay), (bx, by) = out["direct"], out["lattice"]
+        assert np.array_equal(bx, out["lattice_incta"][0]) and np.array_equal(by, out["lattice_incta"][1]), case
         assert np.all(np.isfinite(bx)) and np.all(np.isfinite(by)), case
         s = max(np.abs(ax).max(), np.abs(ay).max())
         worst = max(worst, max(np.abs(ax - bx).max(), np.abs(ay - by).max()) / s)

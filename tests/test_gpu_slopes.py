@@ -20,9 +20,10 @@ def torch_cuda():
     return torch
 
 
-def gpu_force_linear(torch, lay, sigma, dx, dy, then_zeroth=False):
+def gpu_force_linear(torch, lay, sigma, dx, dy, then_zeroth=False, mode="direct"):
     from paper_2001_02765_b200 import SgDisk
     with SgDisk.from_layout(lay, device=0) as d:
+        d.set_interaction_mode(mode)
         t = [torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda() for a in (sigma, dx, dy)]
         d.set_density_linear(*t)
         Fx, Fy = d.force()
@@ -77,20 +78,89 @@ def test_nested_five_levels_vs_oracle(torch_cuda):
     assert emax <= 1e-11 and l2 <= 1e-12, (emax, l2)
 
 
-def test_galactic_config_sampled_vs_oracle(torch_cuda):
+@pytest.mark.parametrize("mode", ["direct", "lattice"])
+def test_galactic_config_sampled_vs_oracle(torch_cuda, mode):
     """cfg 3 (53,248 leaves, 4 levels, lattice extent 2048) with centred-difference-free analytic slopes of a
-    smooth bump; oracle on 1024 sampled targets."""
+    smooth bump; oracle on 1024 sampled targets.  lattice: three-plane function lattices for the pairs <= 2 levels
+    apart, direct slope sums for the level 0 <-> level 3 pairs (patch_far_kernel<true>)."""
     lay, _ = make_config(3)
     x, y, _ = cell_centres(lay)
     s2 = 4.0 ** 2
     sigma = np.exp(-(x * x + y * y) / (2 * s2))
     dx, dy = -x / s2 * sigma, -y / s2 * sigma
-    gx, gy = gpu_force_linear(torch_cuda, lay, sigma, dx, dy)
+    gx, gy = gpu_force_linear(torch_cuda, lay, sigma, dx, dy, mode=mode)
     idx = sample_targets(lay, 1024, 77)
     r = cell_rects(lay)
     ox, oy, _ = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, dx=dx, dy=dy)
     emax, l2 = errors(gx[idx], gy[idx], ox, oy)
     assert emax <= 1e-11 and l2 <= 1e-12, (emax, l2)
+
+
+# ------------------------------------------------------------------------------------------
+# slope path in lattice mode (SURVEY.md 8 f1 x f2): same tolerances as the direct slope kernel
+# ------------------------------------------------------------------------------------------
+def _lattice_slopes_vs_oracle(torch, lay, sigma, dx, dy, idx=None):
+    from paper_2001_02765_b200 import SgDisk
+    if idx is None:
+        idx = np.arange(lay.n_cells)
+    r = cell_rects(lay)
+    ox, oy, _ = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, dx=dx, dy=dy)
+    with SgDisk.from_layout(lay, device=0) as d:
+        t = [torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda() for a in (sigma, dx, dy)]
+        d.set_interaction_mode("lattice")
+        d.set_density_linear(*t)
+        assert d.kernel_model()["fp64_instr_per_pair"] == 6.0       # the lattice slope path is the one that runs
+        Fx, Fy = d.force()
+        d.set_interaction_mode("direct")
+        Dx, Dy = d.force()
+        d.set_interaction_mode("lattice")
+        Gx, Gy = d.force()                                           # again, after a mode change: bit-identical
+        torch.cuda.synchronize()
+        assert torch.equal(Fx, Gx) and torch.equal(Fy, Gy)
+    gx, gy = Fx.cpu().numpy(), Fy.cpu().numpy()
+    assert np.all(np.isfinite(gx)) and np.all(np.isfinite(gy))
+    emax, l2 = errors(gx[idx], gy[idx], ox, oy)
+    assert emax <= 1e-11 and l2 <= 1e-12, (emax, l2)
+    s = max(np.abs(ox).max(), np.abs(oy).max())
+    assert max(np.abs(gx - Dx.cpu().numpy()).max(), np.abs(gy - Dy.cpu().numpy()).max()) <= 1e-11 * s
+    return gx, gy
+
+
+def test_lattice_slopes_two_level_patches_all_targets(torch_cuda):
+    """cfg-2-shaped two-level AMR with 16 x 16 patches (coarse ring + refined centre), noisy sigma, Taylor slopes of the
+    smooth profile: all 12,288 targets vs the oracle's first-order sum."""
+    lay = nested_layout(2, 128, 1.0, 16)
+    x, y, _ = cell_centres(lay)
+    sigma = kuzmin_sigma(x, y) * (1 + 0.05 * np.random.default_rng(1).uniform(-1, 1, lay.n_cells))
+    _lattice_slopes_vs_oracle(torch_cuda, lay, sigma, *kuzmin_slopes(x, y))
+
+
+def test_lattice_slopes_five_nested_levels_all_targets(torch_cuda):
+    """Five nested levels, P = 16: every pair class by function lattices and the pairs three and four levels apart by
+    the direct slope sum (patch_far_kernel<true>)."""
+    lay = nested_layout(5, 64, 8.0, 16)
+    x, y, _ = cell_centres(lay)
+    _lattice_slopes_vs_oracle(torch_cuda, lay, kuzmin_sigma(x, y, a=0.7), *kuzmin_slopes(x, y, a=0.7))
+
+
+def test_lattice_slopes_irregular_hierarchy(torch_cuda):
+    """Ragged three-level hierarchy with holes (workloads.random_refined_layout), all targets."""
+    from workloads import random_refined_layout
+    lay = random_refined_layout(3, 6, 16, 3, 0.3)
+    x, y, _ = cell_centres(lay)
+    _lattice_slopes_vs_oracle(torch_cuda, lay, kuzmin_sigma(x, y, a=0.4), *kuzmin_slopes(x, y, a=0.4))
+
+
+def test_lattice_slopes_config4_sampled(torch_cuda):
+    """BASELINE.json config 4 (three levels, 448,768 leaves) with the slopes of its own smooth profile taken by centred
+    differences of the formula; 512 stratified targets."""
+    from workloads.configs import _ppd_sigma
+    lay, sigma = make_config(4)
+    x, y, h = cell_centres(lay)
+    e = 1e-4
+    dx = (_ppd_sigma(x + e, y) - _ppd_sigma(x - e, y)) / (2 * e)
+    dy = (_ppd_sigma(x, y + e) - _ppd_sigma(x, y - e)) / (2 * e)
+    _lattice_slopes_vs_oracle(torch_cuda, lay, sigma, dx, dy, idx=sample_targets(lay, 512, 4004))
 
 
 def test_random_slopes_conditioning(torch_cuda):
@@ -107,6 +177,21 @@ def test_random_slopes_conditioning(torch_cuda):
 
 
 _d2_uniform_cache = {}
+
+
+def test_paper_table1_row_1024_in_lattice_mode(torch_cuda, golden):
+    """PAPER.md:152 (Table 1, N_k = 1024) from the lattice-mode slope path: the paper's full second-order method on its
+    own 1024^2 grid in ~0.55 s (171 s on the paper's P100)."""
+    row = [r for r in golden("paper_table1_D2_uniform.txt") if int(r[0]) == 1024][0]
+    lay = uniform_layout(1024, -1.0, -1.0, 2 / 1024, 16)
+    x, y, h = cell_centres(lay)
+    Fx, Fy = gpu_force_linear(torch_cuda, lay, d2_sigma(x, y, 0.5), *d2_slopes(x, y, 0.5), mode="lattice")
+    ax, ay = F_D2_xy(x, y, 0.5)
+    R = np.hypot(x, y)
+    eR = (Fx * x + Fy * y) / R - (ax * x + ay * y) / R
+    got = list(_norms(Fx - ax, h ** 2)) + list(_norms(eR, h ** 2))
+    for g, p in zip(got, row[1:]):
+        assert _agree_3_digits(g, p), (got, row)
 
 
 def d2_uniform_gpu(torch, Nk):
