@@ -36,6 +36,12 @@ struct sg_ctx {
     LatticeArrays lat;           // precomputed function lattices of the pair classes (sg_kernels_lattice.cu)
     std::vector<FnLattice> lat_meta;        // host copy, [n_levels * kOffClasses]
     int64_t lat_entries = 0;                // entries per plane; 0: no plan (P != 16) or over the memory budget
+    // regrouped lattice mode (P = 1, 2 or 4, e.g. the paper's zone-wise quadtrees): the leaves are packed into padded
+    // 16 x 16 blocks of an inner context that runs the lattice kernels; cell data is permuted in and out
+    sg_ctx *inner = nullptr;
+    int32_t *rg_map = nullptr, *rg_inv = nullptr;       // device: caller cell -> inner cell; inner cell -> caller cell or -1
+    double *rg_in[3] = {nullptr, nullptr, nullptr};     // sigma, dx, dy in inner cell order
+    double *rg_f[2] = {nullptr, nullptr};               // Fx, Fy in inner cell order
     int64_t first = 0, count = 0;
     int64_t dev_bytes = 0;
     std::vector<void *> allocs;
@@ -582,13 +588,13 @@ int upload_layout(sg_ctx *c) {
 
 extern "C" {
 
-int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, double y0, int patch_cells,
-              const sg_patch *leaf_patches, int64_t n_patches, double G, int device) {
+static int create_ctx(sg_ctx **out, int n_levels, const double *cell_width, double x0, double y0, int patch_cells,
+                      const sg_patch *leaf_patches, int64_t n_patches, double G, int device, const uint8_t *cell_present) {
     if (!out) { g_create_error = "out is NULL"; return SG_ERR_ARG; }
     *out = nullptr;
     if (!std::isfinite(G)) { g_create_error = "G must be finite"; return SG_ERR_ARG; }
     sg_ctx *c = new sg_ctx();
-    int rc = build_layout(c->host, n_levels, cell_width, x0, y0, patch_cells, leaf_patches, n_patches, c->err);
+    int rc = build_layout(c->host, n_levels, cell_width, x0, y0, patch_cells, leaf_patches, n_patches, c->err, cell_present);
     if (rc == SG_OK) {
         c->device = device;
         c->dev.G = G;
@@ -617,8 +623,71 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
     return SG_OK;
 }
 
+int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, double y0, int patch_cells,
+              const sg_patch *leaf_patches, int64_t n_patches, double G, int device) {
+    return create_ctx(out, n_levels, cell_width, x0, y0, patch_cells, leaf_patches, n_patches, G, device, nullptr);
+}
+
+// Regrouping for lattice mode (P = 1, 2, 4): every leaf cell of level l at (ci, cj) on its level's lattice goes to
+// the aligned 16 x 16 block (l, ci >> 4, cj >> 4); a block that is only partly covered by leaves of its level is
+// padded with holes (targets whose result is discarded, no sources: build_layout's cell_present).  The inner context
+// is an ordinary P = 16 context on that padded layout.
+static int build_regrouped(sg_ctx *c) {
+    const HostLayout &h = c->host;
+    const int P = h.P;
+    std::vector<uint64_t> keys(size_t(h.N));
+    std::vector<uint32_t> within(size_t(h.N));
+    {
+        int64_t cell = 0;
+        for (size_t p = 0; p < h.patches.size(); ++p) {
+            const sg_patch &q = h.patches[p];
+            for (int j = 0; j < P; ++j)
+                for (int i = 0; i < P; ++i, ++cell) {
+                    const uint64_t ci = uint64_t(q.i0 + i), cj = uint64_t(q.j0 + j);
+                    keys[size_t(cell)] = (uint64_t(q.level) << 56) | ((cj >> 4) << 28) | (ci >> 4);   // sorts by (level, bj, bi)
+                    within[size_t(cell)] = uint32_t((cj & 15) * 16 + (ci & 15));
+                }
+        }
+    }
+    std::vector<uint64_t> blocks(keys);
+    std::sort(blocks.begin(), blocks.end());
+    blocks.erase(std::unique(blocks.begin(), blocks.end()), blocks.end());
+    const int64_t nb = int64_t(blocks.size()), n_inner = nb * 256;
+    if (n_inner >= (int64_t(1) << 29)) { c->err = "regrouped layout too large"; return SG_ERR_LAYOUT; }
+    std::vector<sg_patch> bp;
+    bp.resize(size_t(nb));
+    for (int64_t b = 0; b < nb; ++b) {
+        const uint64_t k = blocks[size_t(b)];
+        bp[size_t(b)] = sg_patch{int32_t(k >> 56), int32_t((k & 0xfffffffu) * 16), int32_t(((k >> 28) & 0xfffffffu) * 16)};
+    }
+    std::vector<int32_t> map(size_t(h.N)), inv(size_t(n_inner), -1);
+    std::vector<uint8_t> present(size_t(n_inner), 0);
+    for (int64_t cell = 0; cell < h.N; ++cell) {
+        const int64_t b = std::lower_bound(blocks.begin(), blocks.end(), keys[size_t(cell)]) - blocks.begin();
+        const int64_t k = b * 256 + within[size_t(cell)];
+        map[size_t(cell)] = int32_t(k);
+        inv[size_t(k)] = int32_t(cell);
+        present[size_t(k)] = 1;
+    }
+    std::vector<double> cw(size_t(h.n_levels));
+    for (int l = 0; l < h.n_levels; ++l) cw[size_t(l)] = h.unit * double(int64_t(2) << (h.n_levels - 1 - l));
+    sg_ctx *in = nullptr;
+    int rc = create_ctx(&in, h.n_levels, cw.data(), h.x0, h.y0, 16, bp.data(), nb, c->dev.G, c->device, present.data());
+    if (rc != SG_OK) { c->err = "regrouped layout: " + g_create_error; return rc; }
+    c->inner = in;
+    if ((rc = upload(c, &c->rg_map, map)) || (rc = upload(c, &c->rg_inv, inv))) return rc;
+    for (int k = 0; k < 3; ++k)
+        if ((rc = dev_alloc(c, &c->rg_in[k], n_inner))) return rc;
+    for (int k = 0; k < 2; ++k)
+        if ((rc = dev_alloc(c, &c->rg_f[k], n_inner))) return rc;
+    return SG_OK;
+}
+
+static bool regroupable(const sg_ctx *c) { return c->host.P == 1 || c->host.P == 2 || c->host.P == 4; }
+
 void sg_destroy(sg_ctx *c) {
     if (!c) return;
+    if (c->inner) { sg_destroy(c->inner); c->inner = nullptr; }
     if (c->device >= 0) {
         DeviceGuard guard(c->device);
         cudaDeviceSynchronize();
@@ -641,7 +710,7 @@ int sg_layout_info(const sg_ctx *c, int64_t *info) {
     info[2] = int64_t(c->host.colX.size()); info[3] = int64_t(c->host.rowY.size());
     info[4] = int64_t(c->host.tX.size()); info[5] = int64_t(c->host.tY.size());
     info[6] = c->host.balanced ? 1 : 0;
-    info[7] = c->dev_bytes;
+    info[7] = c->dev_bytes + (c->inner ? c->inner->dev_bytes : 0);
     return SG_OK;
 }
 
@@ -670,6 +739,11 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = false;
+    if (c->inner) {                                           // regrouped lattice mode: the same sigma in block order
+        launch_scatter_cells(sigma_dev, nullptr, nullptr, c->rg_inv, c->rg_in[0], nullptr, nullptr, c->inner->host.N, s);
+        const int rc = sg_set_density(c->inner, c->rg_in[0], cuda_stream);
+        if (rc) { c->err = c->inner->err; return rc; }
+    }
     return SG_OK;
 }
 
@@ -708,6 +782,11 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = true;
+    if (c->inner) {
+        launch_scatter_cells(sigma_dev, dx_dev, dy_dev, c->rg_inv, c->rg_in[0], c->rg_in[1], c->rg_in[2], c->inner->host.N, s);
+        const int rc = sg_set_density_linear(c->inner, c->rg_in[0], c->rg_in[1], c->rg_in[2], cuda_stream);
+        if (rc) { c->err = c->inner->err; return rc; }
+    }
     return SG_OK;
 }
 
@@ -720,6 +799,18 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     DeviceGuard guard(c->device);
     SG_CUDA(c, guard.err);
+    if (c->use_patch && c->inner) {
+        // regrouped lattice mode: the inner context evaluates every block, the caller's targets are picked out of it
+        if (!c->inner->density_set || c->inner->linear != c->linear) {
+            c->err = "regrouped lattice mode: set the density after sg_set_interaction_mode(SG_MODE_LATTICE)";
+            return SG_ERR_STATE;
+        }
+        const int rc = sg_force(c->inner, c->rg_f[0], c->rg_f[1], cuda_stream);
+        if (rc) { c->err = c->inner->err; return rc; }
+        launch_gather_cells(c->rg_f[0], c->rg_f[1], c->rg_map, c->first, c->count, Fx_dev, Fy_dev, s);
+        SG_CUDA(c, cudaGetLastError());
+        return SG_OK;
+    }
     const StepPlan sp = make_step_plan(c, c->linear);
     const ForcePlan &p = sp.p;
     int rc = grow_partials(c, sp.partials(), s);           // no-op: reserve_partials() sized it (fallback otherwise)
@@ -815,8 +906,22 @@ int sg_set_interaction_mode(sg_ctx *c, int mode) {
     if (mode != SG_MODE_DIRECT && mode != SG_MODE_LATTICE && mode != SG_MODE_LATTICE_BLOCKED && mode != SG_MODE_LATTICE_INCTA) {
         c->err = "unknown interaction mode"; return SG_ERR_ARG;
     }
+    if (mode == SG_MODE_LATTICE && regroupable(c) && c->device >= 0) {
+        // small patches (the paper's zone-wise quadtrees): pack the leaves into padded 16 x 16 blocks once
+        DeviceGuard guard(c->device);
+        SG_CUDA(c, guard.err);
+        if (!c->inner) {
+            const int rc = build_regrouped(c);
+            if (rc) return rc;
+        }
+        const int rc = sg_set_interaction_mode(c->inner, SG_MODE_LATTICE);
+        if (rc) { c->err = c->inner->err; return rc; }
+        c->use_patch = true;
+        return SG_OK;
+    }
     if (mode == SG_MODE_LATTICE && c->host.P != 8 && c->host.P != 16) {
-        c->err = "SG_MODE_LATTICE needs patches of 8 x 8 or 16 x 16 cells"; return SG_ERR_ARG;
+        c->err = "SG_MODE_LATTICE needs patches of 8 x 8 or 16 x 16 cells (or of 1, 2 or 4 cells, regrouped on a device)";
+        return SG_ERR_ARG;
     }
     if ((mode == SG_MODE_LATTICE_BLOCKED || mode == SG_MODE_LATTICE_INCTA) &&
         (c->host.P != 16 || (c->device >= 0 && !c->patch.blocked))) {
@@ -906,6 +1011,18 @@ int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
 
 int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     if (!c) return SG_ERR_ARG;
+    if (c->inner) {                                               // + the permutation kernels
+        int a = 0, b = 0, a2 = 0, b2 = 0;
+        sg_launch_counts(c->inner, &a, &b);
+        sg_ctx *mut = const_cast<sg_ctx *>(c);                    // own counts as if there were no inner context
+        sg_ctx *saved = mut->inner;
+        mut->inner = nullptr;
+        sg_launch_counts(c, &a2, &b2);
+        mut->inner = saved;
+        if (set_density_launches) *set_density_launches = a2 + 1 + a;
+        if (force_launches) *force_launches = c->use_patch ? (c->count > 0 ? b + 1 : 0) : b2;
+        return SG_OK;
+    }
     // vertex weights, running sums and look-ups per direction (+ per-patch weights when the lattice-offset path exists);
     // with slopes: weights, column tables, row tables (+ per-patch slope weights)
     if (set_density_launches) *set_density_launches = c->linear ? 3 + (c->lat.wS ? 1 : 0) : 5 + (c->patch.enabled ? 1 : 0);
@@ -922,6 +1039,10 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
 
 int sg_set_kernel_timing(sg_ctx *c, int enable) {
     if (!c) return SG_ERR_ARG;
+    if (c->inner) {
+        const int rc = sg_set_kernel_timing(c->inner, enable);
+        if (rc) { c->err = c->inner->err; return rc; }
+    }
     if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
     DeviceGuard guard(c->device);
     SG_CUDA(c, guard.err);
@@ -940,6 +1061,7 @@ int sg_set_kernel_timing(sg_ctx *c, int enable) {
 int sg_get_kernel_times(sg_ctx *c, float *ms, int capacity, int *n) {
     if (!c || !ms || !n || capacity < 0) return SG_ERR_ARG;
     *n = 0;
+    if (c->inner && c->use_patch) return sg_get_kernel_times(c->inner, ms, capacity, n);
     if (c->device < 0) { c->err = "host-only context"; return SG_ERR_CUDA; }
     const int64_t have = std::min<int64_t>(c->timed_calls, kTimingRing);
     const int64_t take = std::min<int64_t>(have, capacity);
@@ -961,6 +1083,8 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
     // algorithmic unit: one (target, deduplicated vertex) pair; one launch processes count * N_v
     const double alg = double(c->count) * double(c->host.Nv);
     if (pair_evaluations) *pair_evaluations = alg;
+    if (c->inner && c->use_patch)                                 // regrouped: the blocks' work, the caller's units
+        return sg_kernel_model(c->inner, fp64_instr_per_pair, flops_per_pair, nullptr, executed_evaluations);
     const StepPlan sp = make_step_plan(c, c->linear);
     if (sp.by_patch && c->linear) {
         // slope path in lattice mode: three planes, 6 DFMA per pair (sg_kernels_lattice.cu)

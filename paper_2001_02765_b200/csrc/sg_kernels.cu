@@ -342,6 +342,41 @@ void launch_finalise(const DevLayout &d, const ForcePlan &p, double *Fx, double 
 }
 
 // ------------------------------------------------------------------------------------------------
+// Regrouped layouts (small patches packed into padded 16 x 16 blocks for lattice mode, sg_api.cu): cell data of the
+// caller's order <-> the block order of the inner context.  inv[k] = caller cell of inner cell k, or -1 (hole).
+// ------------------------------------------------------------------------------------------------
+__global__ void scatter_cells_kernel(const double *__restrict__ a, const double *__restrict__ b,
+                                     const double *__restrict__ c, const int32_t *__restrict__ inv,
+                                     double *__restrict__ oa, double *__restrict__ ob, double *__restrict__ oc,
+                                     int64_t n_inner) {
+    const int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (k >= n_inner) return;
+    const int32_t s = inv[k];
+    oa[k] = s >= 0 ? a[s] : 0.0;
+    if (b) { ob[k] = s >= 0 ? b[s] : 0.0; oc[k] = s >= 0 ? c[s] : 0.0; }
+}
+
+__global__ void gather_cells_kernel(const double *__restrict__ fx, const double *__restrict__ fy,
+                                    const int32_t *__restrict__ map, int64_t first, int64_t count,
+                                    double *__restrict__ ox, double *__restrict__ oy) {
+    const int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const int32_t k = map[first + i];
+    ox[i] = fx[k];
+    oy[i] = fy[k];
+}
+
+void launch_scatter_cells(const double *a, const double *b, const double *c, const int32_t *inv, double *oa, double *ob,
+                          double *oc, int64_t n_inner, cudaStream_t s) {
+    scatter_cells_kernel<<<unsigned((n_inner + 255) / 256), 256, 0, s>>>(a, b, c, inv, oa, ob, oc, n_inner);
+}
+
+void launch_gather_cells(const double *fx, const double *fy, const int32_t *map, int64_t first, int64_t count,
+                         double *ox, double *oy, cudaStream_t s) {
+    if (count > 0) gather_cells_kernel<<<unsigned((count + 255) / 256), 256, 0, s>>>(fx, fy, map, first, count, ox, oy);
+}
+
+// ------------------------------------------------------------------------------------------------
 // FP64 peak: 8 independent DFMA chains per thread, 4 CTAs of 256 threads per SM.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) dfma_kernel(double *out, int iters, double a, double b) {

@@ -30,7 +30,7 @@ void sorted_unique(std::vector<int32_t> &v) {
 }  // namespace
 
 int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x0, double y0, int P,
-                 const sg_patch *patches, int64_t n_patches, std::string &err) {
+                 const sg_patch *patches, int64_t n_patches, std::string &err, const uint8_t *cell_present) {
     if (!cell_width || !patches) { err = "null pointer argument"; return SG_ERR_ARG; }
     if (n_levels < 1 || n_levels > 24) { err = "n_levels must be in 1..24"; return SG_ERR_ARG; }
     if (P < 1 || P > 4096) { err = "patch_cells must be in 1..4096"; return SG_ERR_ARG; }
@@ -76,7 +76,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
             if (leafset.count(patch_key(l, pi, pj))) return l;                // at `level` and coarser
         return -1;
     };
-    for (int64_t p = 0; p < n_patches; ++p) {
+    for (int64_t p = 0; p < n_patches && !cell_present; ++p) {
         const sg_patch &q = patches[p];
         const int64_t pi = q.i0 / P, pj = q.j0 / P;
         if (q.level > 0 && covering_level(q.level - 1, pi >> 1, pj >> 1) >= 0) {
@@ -116,7 +116,8 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     // ---- vertices: sort the 4N (corner key, cell, corner) records, merge equal keys ------------
     // corner id: 0 = NE (+), 1 = NW (-), 2 = SE (-), 3 = SW (+)
     struct Rec { uint64_t key; uint32_t cc; };
-    std::vector<Rec> rec(size_t(N) * 4);
+    std::vector<Rec> rec;
+    rec.reserve(size_t(N) * 4);
     {
         int64_t c = 0;
         for (int64_t p = 0; p < n_patches; ++p) {
@@ -124,15 +125,17 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
             const int32_t cw = int32_t(2) << (n_levels - 1 - q.level);
             for (int j = 0; j < P; ++j)
                 for (int i = 0; i < P; ++i, ++c) {
+                    if (cell_present && !cell_present[c]) continue;       // a hole of a padded layout: not a source
                     const uint64_t xl = uint64_t(q.i0 + i) * cw, xr = xl + cw;
                     const uint64_t yd = uint64_t(q.j0 + j) * cw, yu = yd + cw;
-                    rec[4 * c + 0] = {(xr << 32) | yu, uint32_t(c << 2) | 0u};
-                    rec[4 * c + 1] = {(xl << 32) | yu, uint32_t(c << 2) | 1u};
-                    rec[4 * c + 2] = {(xr << 32) | yd, uint32_t(c << 2) | 2u};
-                    rec[4 * c + 3] = {(xl << 32) | yd, uint32_t(c << 2) | 3u};
+                    rec.push_back({(xr << 32) | yu, uint32_t(c << 2) | 0u});
+                    rec.push_back({(xl << 32) | yu, uint32_t(c << 2) | 1u});
+                    rec.push_back({(xr << 32) | yd, uint32_t(c << 2) | 2u});
+                    rec.push_back({(xl << 32) | yd, uint32_t(c << 2) | 3u});
                 }
         }
     }
+    if (rec.empty()) { err = "no leaf cell present"; return SG_ERR_ARG; }
     std::sort(rec.begin(), rec.end(), [](const Rec &a, const Rec &b) {
         return a.key != b.key ? a.key < b.key : a.cc < b.cc;
     });
@@ -197,7 +200,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
         vset.reserve(size_t(L.Nv) * 2);
         for (int64_t v = 0; v < L.Nv; ++v) vset.insert((uint64_t(L.vkx[v]) << 32) | uint32_t(L.vky[v]));
         for (int64_t c = 0; c < N; ++c)
-            if (vset.count((uint64_t(L.tkx[c]) << 32) | uint32_t(L.tky[c]))) {
+            if ((!cell_present || cell_present[c]) && vset.count((uint64_t(L.tkx[c]) << 32) | uint32_t(L.tky[c]))) {
                 err = fmt("cell %lld: centre coincides with a vertex of another leaf: leaves overlap", c);
                 return SG_ERR_LAYOUT;
             }

@@ -48,7 +48,13 @@ constexpr int kChunk = 16;                 // vertices per chunk
 constexpr int kChunksPerTile = 16;         // chunks per shared-memory tile (one TMA bulk copy)
 
 // Returns SG_OK or SG_ERR_*; on error `err` holds the message.
+// cell_present (optional, [n_patches * P * P], library cell order): a PADDED layout, used internally when a layout of
+// small patches is regrouped into 16 x 16 blocks for lattice mode -- cells with 0 are holes (the block is only partly
+// covered by leaves of its level): they are targets whose result is discarded and they are not sources (no vertex
+// records, no adjacency), so patches of different levels may overlap in their holes and the overlap / balance checks
+// are skipped (the layout was derived from one that passed them).
 int build_layout(HostLayout &out, int n_levels, const double *cell_width, double x0, double y0,
-                 int P, const sg_patch *patches, int64_t n_patches, std::string &err);
+                 int P, const sg_patch *patches, int64_t n_patches, std::string &err,
+                 const uint8_t *cell_present = nullptr);
 
 }  // namespace sg

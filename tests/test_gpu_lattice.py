@@ -247,12 +247,16 @@ def test_fuzz_random_hierarchies_lattice_vs_direct(torch_cuda):
 
 def test_unsupported_patch_size_is_refused(torch_cuda):
     from paper_2001_02765_b200 import SgDisk, SgError, binding
-    lay = paper_ilr_layout(32, 2)                                  # P = 1 quadtree
+    lay = Layout(1, np.array([0.125]), -1.0, -1.0, 3, np.array([[0, 0, 0], [0, 3, 0]], dtype=np.int32))   # P = 3
     with SgDisk.from_layout(lay, device=0) as d:
         with pytest.raises(SgError) as e:
             d.set_interaction_mode("lattice")
         assert e.value.code == binding.SG_ERR_ARG
         d.set_interaction_mode("direct")
+    with SgDisk.from_layout(paper_ilr_layout(32, 2), device=0) as d:       # P = 1: regrouped, but no in-CTA variant
+        d.set_interaction_mode("lattice")
+        with pytest.raises(SgError):
+            d.set_interaction_mode("lattice_blocked")
     lay2, _ = make_config(2)                                       # P = 8: generic lattice kernel only
     with SgDisk.from_layout(lay2, device=0) as d:
         d.set_interaction_mode("lattice")
@@ -276,3 +280,91 @@ def test_cost_based_rank_slices_concatenate_to_the_full_result(torch_cuda):
         gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice", target_range=(first, count))
         px.append(gx); py.append(gy)
     assert np.array_equal(np.concatenate(px), fx) and np.array_equal(np.concatenate(py), fy)
+
+
+# ------------------------------------------------------------------------------------------
+# regrouped lattice mode: layouts of 1 x 1, 2 x 2 or 4 x 4 patches (the paper's zone-wise quadtrees) packed into padded
+# 16 x 16 blocks of an inner context (sg_api.cu build_regrouped)
+# ------------------------------------------------------------------------------------------
+def _regrouped_case(name):
+    from workloads.configs import _sorted_patches
+    if name == "ilr":                                              # PAPER.md:164 ILR quadtree, three levels
+        lay = paper_ilr_layout(64, 3)
+    elif name == "fig1":                                           # PAPER.md:110 Fig. 1 / Table 10: 28 leaves, unbalanced
+        l0 = [(0, i, j) for j in range(4) for i in range(4) if (i, j) not in ((1, 1), (2, 2))]
+        l1 = [(1, 2, 2), (1, 3, 3)] + [(1, 4 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]
+        l2 = [(2, 4 + di, 6 + dj) for dj in (0, 1) for di in (0, 1)]
+        l2 += [(2, 6 + di, 4 + dj) for dj in (0, 1) for di in (0, 1)]
+        lay = Layout(3, np.array([0.25, 0.125, 0.0625]), 0.0, 0.0, 1, _sorted_patches(l0 + l1 + l2))
+    elif name == "nest_p4":                                        # five nested levels of 4 x 4 patches (far pairs)
+        lay = nested_layout(5, 32, 8.0, 4)
+    else:                                                          # ragged hierarchy of 2 x 2 patches
+        lay = random_refined_layout(11, 24, 2, 4, 0.3)
+    return lay
+
+
+@pytest.mark.parametrize("name", ["ilr", "fig1", "nest_p4", "rand_p2"])
+def test_regrouped_small_patches_vs_oracle(torch_cuda, name):
+    lay = _regrouped_case(name)
+    sigma = _noisy_kuzmin(lay, 90)
+    gx, gy = gpu_force(torch_cuda, lay, sigma, "lattice")
+    check(gx, gy, *oracle_force(lay, sigma, np.arange(lay.n_cells)))
+    dx, dy = gpu_force(torch_cuda, lay, sigma, "direct")
+    s = max(np.abs(dx).max(), np.abs(dy).max())
+    assert max(np.abs(gx - dx).max(), np.abs(gy - dy).max()) <= 1e-12 * s
+    n = lay.n_cells
+    for first, count in ((0, 1), (n // 3, n // 2), (n - 1, 1), (5, 0)):
+        rx, ry = gpu_force(torch_cuda, lay, sigma, "lattice", target_range=(first, count))
+        assert rx.shape == (count,)
+        assert np.array_equal(rx, gx[first:first + count]) and np.array_equal(ry, gy[first:first + count])
+
+
+def test_regrouped_mode_state_and_mode_switches(torch_cuda):
+    """Density set before lattice mode was selected on a small-patch layout: sg_force refuses (SG_ERR_STATE) instead of
+    using a stale inner density; after set_density both modes work on one context, any order."""
+    from paper_2001_02765_b200 import SgDisk, SgError, binding
+    lay = paper_ilr_layout(64, 2)
+    sigma = _noisy_kuzmin(lay, 91)
+    with SgDisk.from_layout(lay, device=0) as d:
+        s = torch_cuda.as_tensor(sigma).cuda()
+        d.set_density(s)
+        ref = [t.cpu().numpy() for t in d.force()]
+        d.set_interaction_mode("lattice")
+        with pytest.raises(SgError) as e:
+            d.force()
+        assert e.value.code == binding.SG_ERR_STATE
+        d.set_density(s)
+        a = [t.cpu().numpy() for t in d.force()]
+        d.set_interaction_mode("direct")
+        b = [t.cpu().numpy() for t in d.force()]
+        d.set_interaction_mode("lattice")
+        c = [t.cpu().numpy() for t in d.force()]
+    sc = max(np.abs(ref[0]).max(), np.abs(ref[1]).max())
+    assert np.array_equal(b[0], ref[0]) and np.array_equal(a[0], c[0]) and np.array_equal(a[1], c[1])
+    assert max(np.abs(a[0] - ref[0]).max(), np.abs(a[1] - ref[1]).max()) <= 1e-12 * sc
+
+
+def test_regrouped_paper_quadtree_at_scale(torch_cuda):
+    """AMR(3, D2) at N_k = 1024 (1,419,424 leaves, Table 8: 1,050 s on the paper's P100 with slopes): the
+    zeroth-order sum in regrouped lattice mode against the direct kernel everywhere and the oracle on 96 targets."""
+    from paper_2001_02765_b200 import SgDisk
+    from workloads import d2_sigma
+    lay = paper_ilr_layout(1024, 3)
+    x, y, _ = cell_centres(lay)
+    sigma = d2_sigma(x, y, 0.5)
+    with SgDisk.from_layout(lay, device=0) as d:
+        s = torch_cuda.as_tensor(sigma).cuda()
+        d.set_interaction_mode("lattice")
+        d.set_density(s)
+        d.force()
+        d.set_kernel_timing(True)
+        gx, gy = [t.cpu().numpy() for t in d.force()]
+        t_lat = d.kernel_times_ms()[-1]
+        d.set_interaction_mode("direct")
+        dx, dy = [t.cpu().numpy() for t in d.force()]
+        t_dir = d.kernel_times_ms()[-1]
+    sc = max(np.abs(dx).max(), np.abs(dy).max())
+    assert max(np.abs(gx - dx).max(), np.abs(gy - dy).max()) <= 1e-12 * sc
+    assert t_dir >= 5.0 * t_lat, (t_dir, t_lat)                    # VERDICT r1 item 7: >= 5x the direct time
+    idx = sample_targets(lay, 96, 3071)
+    check(gx[idx], gy[idx], *oracle_force(lay, sigma, idx))

@@ -319,8 +319,6 @@ def test_P2_paper_tables4_6_D22_Linf(golden, rule, L, Nk):
 
 def test_paper_leaf_counts_tables_8_9(golden):
     for rule, disk, L, Nk, EL in golden("paper_table8_9_leaf_counts.txt"):
-        if int(Nk) > 256:
-            continue
         f = paper_ilr_layout if rule == "ILR" else paper_vlr_layout
         assert f(int(Nk), int(L), disk).n_cells == int(EL), (rule, disk, L, Nk)
 

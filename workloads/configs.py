@@ -327,23 +327,30 @@ def _paper_band_layout(Nk: int, L: int, centres, alpha: float, band_of_level) ->
     refined iff | R_c - alpha | < band_of_level(m+1) with R_c measured from the nearest disk centre.
     Reading A13/A14 of SURVEY.md section 8(c), pinned against the zone counts of Tables 8 and 9."""
     h1 = 2.0 / Nk
-    zones = [(0, i, j) for j in range(Nk) for i in range(Nk)]
+    jj, ii = np.meshgrid(np.arange(Nk, dtype=np.int64), np.arange(Nk, dtype=np.int64), indexing="ij")
+    arr = np.stack([np.zeros(Nk * Nk, dtype=np.int64), ii.reshape(-1), jj.reshape(-1)], axis=1)   # (level, i, j)
     leaves = []
     for m in range(1, L + 1):                       # paper level m == our level m-1
         l = m - 1
         h = h1 / 2 ** l
-        arr = np.asarray(zones, dtype=np.int64).reshape(-1, 3)
         if m == L:
-            leaves.extend(map(tuple, arr))
+            leaves.append(arr)
             break
         xc = -1.0 + (arr[:, 1] + 0.5) * h
         yc = -1.0 + (arr[:, 2] + 0.5) * h
         Rc = np.min([np.hypot(xc - cx, yc - cy) for (cx, cy) in centres], axis=0)
         ref = np.abs(Rc - alpha) < band_of_level(m + 1)
-        leaves.extend(map(tuple, arr[~ref]))
+        leaves.append(arr[~ref])
         a = arr[ref]
-        zones = [(l + 1, 2 * i + di, 2 * j + dj) for (_, i, j) in a for dj in (0, 1) for di in (0, 1)]
-    return Layout(L, h1 / 2.0 ** np.arange(L), -1.0, -1.0, 1, _sorted_patches(leaves))
+        # children in the order (dj, di) = (0,0), (0,1), (1,0), (1,1) of every refined zone
+        kids = np.empty((a.shape[0], 4, 3), dtype=np.int64)
+        kids[:, :, 0] = l + 1
+        kids[:, :, 1] = 2 * a[:, None, 1] + np.array([0, 1, 0, 1])
+        kids[:, :, 2] = 2 * a[:, None, 2] + np.array([0, 0, 1, 1])
+        arr = kids.reshape(-1, 3)
+    rows = np.concatenate(leaves, axis=0)
+    order = np.lexsort((rows[:, 1], rows[:, 2], rows[:, 0]))          # sorted by (level, j0, i0)
+    return Layout(L, h1 / 2.0 ** np.arange(L), -1.0, -1.0, 1, rows[order].astype(np.int32))
 
 
 def paper_ilr_layout(Nk: int, L: int, disk: str = "D2") -> Layout:
