@@ -28,6 +28,7 @@ struct sg_ctx {
     std::vector<PatchInfo> patch_info;      // host side of the lattice path (build_patch_plan)
     std::vector<PatchLevel> patch_levels;
     std::vector<int32_t> patch_pmap;
+    std::vector<int32_t> patch_flags;       // per patch: bit 0 row P / bit 1 column P of its vertex lattice carries owned vertices
     bool patch_plan_ok = false;             // P == 16 and the per-level patch maps fit
     std::vector<PatchGroup> patch_groups;   // the three group lists back to back (offset_group_list)
     int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
@@ -253,12 +254,14 @@ int64_t plan_fn_lattices(sg_ctx *c) {
     return total;
 }
 
-// Memory budget of the function lattices (all planes): SG_LATTICE_TABLE_MIB, default 16 GiB.  Over it, lattice mode
-// builds its offset tables inside the CTAs (patch_offset_kernel) and the slope path stays direct.
+// Memory budget of the function lattices (all planes): SG_LATTICE_TABLE_MIB, default a quarter of the device's memory
+// (45 GB on a B200).  Over it, lattice mode builds its offset tables inside the CTAs (patch_offset_kernel) and the
+// slope path stays direct.
 int64_t fn_budget_bytes() {
-    const char *e = std::getenv("SG_LATTICE_TABLE_MIB");
-    const int64_t mib = e ? std::atoll(e) : 16384;
-    return std::max<int64_t>(0, mib) << 20;
+    if (const char *e = std::getenv("SG_LATTICE_TABLE_MIB")) return std::max<int64_t>(0, std::atoll(e)) << 20;
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return int64_t(16) << 30;
+    return int64_t(total_b / 4);
 }
 
 // Build (or extend to the slope planes) the function lattices.  Host-synchronous; no-op when they exist already.
@@ -291,6 +294,16 @@ int ensure_fn_lattices(sg_ctx *c, int n_planes) {
     return SG_OK;
 }
 
+// Source vertices the lattice kernels run through per target: (P + 1)^2 per patch in the generic kernel; in the
+// offset-table kernels (P = 16) vertex row 16 / column 16 of a patch only where it owns vertices there (pflags).
+double executed_patch_vertices(const sg_ctx *c) {
+    const int P = c->host.P;
+    if (c->patch_flags.size() != c->host.patches.size()) return double(c->host.patches.size()) * double((P + 1) * (P + 1));
+    double n = 0.0;
+    for (int32_t f : c->patch_flags) n += double(P + (f & 1)) * double(P + ((f >> 1) & 1));
+    return n;
+}
+
 // Everything one sg_force launches with the current mode and target range.
 struct StepPlan {
     ForcePlan p;                           // direct / slope kernel, and the finalise kernel (p.n_split partial sums per target)
@@ -307,7 +320,8 @@ StepPlan make_step_plan(const sg_ctx *c, bool linear) {
     sp.p = make_plan(c, linear);
     // the slope path runs in lattice mode only through the function lattices (three planes)
     const bool lin_lattice = c->patch.blocked && !c->force_incta && c->lat.n_planes_built >= kFnPlanesLin;
-    sp.by_patch = c->use_patch && (!linear || lin_lattice);
+    // (a regrouped context, c->inner, hands lattice mode to its inner context and plans only its own direct kernels)
+    sp.by_patch = c->use_patch && c->patch.enabled && !c->inner && (!linear || lin_lattice);
     sp.n_planes = linear ? kFnPlanesLin : 1;
     if (sp.by_patch) {
         sp.pp = make_patch_plan(c);
@@ -470,7 +484,11 @@ int upload_patches(sg_ctx *c) {
     if ((rc = upload(c, &pa.info, c->patch_info))) return rc;
     if ((rc = dev_alloc(c, &pa.wP, int64_t(pa.n_patches) * pa.wstride))) return rc;
     {
-        // owner patch of every vertex: the finest patch that has it on its (P+1)^2 lattice, the lowest index among equals
+        // owner patch of every vertex: the finest patch that has it on its (P+1)^2 lattice; among patches of that level
+        // the one that holds it in its lower-left P x P block (i < P and j < P), then i < P, then the lowest index.  On a
+        // uniform level every patch then owns exactly its P x P lower-left vertices, and row P / column P of a patch
+        // carry weights only where no patch of the level continues above / to the right: the offset-table kernels skip
+        // them otherwise (pflags: bit 0 = row P owned somewhere, bit 1 = column P owned in a row below P).
         const int P1 = h.P + 1;
         auto vertex_of = [&](int32_t x, int32_t y) -> int32_t {
             const auto cx = std::lower_bound(h.colX.begin(), h.colX.end(), x);
@@ -481,22 +499,33 @@ int upload_patches(sg_ctx *c) {
             return (it == b1 || *it != y) ? -1 : int32_t(it - h.vky.begin());
         };
         std::vector<int32_t> pv(size_t(pa.n_patches) * P1 * P1, -1), owner(size_t(h.Nv), -1);
+        std::vector<int8_t> owner_rank(size_t(h.Nv), 127);
         for (int p = 0; p < pa.n_patches; ++p) {
             const PatchInfo &q = c->patch_info[size_t(p)];
             for (int j = 0; j < P1; ++j)
                 for (int i = 0; i < P1; ++i) {
                     const int32_t v = vertex_of(q.X0 + i * q.cw, q.Y0 + j * q.cw);
                     pv[(size_t(p) * P1 + j) * P1 + i] = v;
-                    if (v < 0) continue;                           // cannot happen: every patch vertex is a cell corner
+                    if (v < 0) continue;                           // a lattice point of a padded block that no cell touches
+                    const int8_t rank = int8_t((j == h.P ? 2 : 0) + (i == h.P ? 1 : 0));
                     int32_t &o = owner[size_t(v)];
-                    if (o < 0 || c->patch_info[size_t(o)].level < q.level) o = p;
+                    if (o < 0 || c->patch_info[size_t(o)].level < q.level ||
+                        (c->patch_info[size_t(o)].level == q.level && rank < owner_rank[size_t(v)])) {
+                        o = p;
+                        owner_rank[size_t(v)] = rank;
+                    }
                 }
         }
+        std::vector<int32_t> pflags(size_t(pa.n_patches), 0);
         for (int p = 0; p < pa.n_patches; ++p)
             for (int e = 0; e < P1 * P1; ++e) {
                 int32_t &v = pv[size_t(p) * P1 * P1 + e];
                 if (v >= 0 && owner[size_t(v)] != p) v = -1;
+                if (v >= 0 && e / P1 == h.P) pflags[size_t(p)] |= 1;
+                if (v >= 0 && e / P1 < h.P && e % P1 == h.P) pflags[size_t(p)] |= 2;
             }
+        c->patch_flags = pflags;
+        if ((rc = upload(c, &pa.pflags, pflags))) return rc;
         if ((rc = upload(c, &pa.pvmap, pv))) return rc;
     }
     SG_CUDA(c, configure_patch_kernels(pa.P, c->dev.tab_entries));
@@ -1090,8 +1119,7 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
         // slope path in lattice mode: three planes, 6 DFMA per pair (sg_kernels_lattice.cu)
         if (fp64_instr_per_pair) *fp64_instr_per_pair = 6.0;
         if (flops_per_pair) *flops_per_pair = 12.0;
-        if (executed_evaluations)
-            *executed_evaluations = double(c->count) * double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
+        if (executed_evaluations) *executed_evaluations = double(c->count) * executed_patch_vertices(c);
         return SG_OK;
     }
     if (sp.by_patch) {
@@ -1101,8 +1129,7 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
         // directly (21 FP64 instructions each), so the algorithmic fraction is a lower bound on deep hierarchies.
         if (fp64_instr_per_pair) *fp64_instr_per_pair = 2.0;
         if (flops_per_pair) *flops_per_pair = 4.0;
-        if (executed_evaluations)
-            *executed_evaluations = double(c->count) * double(c->host.patches.size()) * double((c->host.P + 1) * (c->host.P + 1));
+        if (executed_evaluations) *executed_evaluations = double(c->count) * executed_patch_vertices(c);
         return SG_OK;
     }
     if (fp64_instr_per_pair) *fp64_instr_per_pair = c->linear ? kLinFp64InstrPerPair : kFp64InstrPerPair;

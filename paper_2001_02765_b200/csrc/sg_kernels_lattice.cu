@@ -97,7 +97,8 @@ template <int V>
 __global__ void __launch_bounds__(kOffWarps * 32, 2)
 lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
-                    const double *__restrict__ wq, int64_t w_plane_stride, const double2 *__restrict__ fn,
+                    const double *__restrict__ wq, int64_t w_plane_stride, const int32_t *__restrict__ pflags,
+                    const double2 *__restrict__ fn,
                     const FnLattice *__restrict__ meta, int n_planes, int n_groups, int n_split, int first_patch,
                     int last_patch, int64_t first, int64_t count, double *__restrict__ part,
                     unsigned int *__restrict__ queue) {
@@ -105,7 +106,6 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     constexpr int P = 16, F = C::F, TROW = C::TROW, TBUF = C::TBUF, K = LatCls<V>::K;
     constexpr int STEP = C::coarser ? F : 1;                              // offsets keep A + d a multiple of F
     constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
-    constexpr int NT = C::finer ? P + F * (kBlkR - 1) + 1 : P + MT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2 *ring = reinterpret_cast<double2 *>(smem_raw);                 // [K][TBUF]
     int *sB = reinterpret_cast<int *>(ring + K * TBUF);                    // [kChunkOffsets][8]
@@ -166,37 +166,10 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
             }
         };
         // correlation of target patch `my_patch` with the vertices of source patch b (weights of plane pl) through
-        // the table T; identical to patch_offset_kernel's (weights through L1)
+        // the table T: correlate_patch, shared with patch_offset_kernel
         auto consume = [&](int b, int pl, const double2 *T) {
             const double2 *src = reinterpret_cast<const double2 *>(wq + int64_t(pl) * w_plane_stride + int64_t(b) * kPatchQStride);
-            if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;   // column F t + this - cc
-            else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
-#pragma unroll 1
-            for (int j = 0; j <= P; ++j) {
-                const double2 *trow = C::coarser ? T + F * j * TROW                                   // row F j - l + 15
-                                                 : T + (j / C::RA + (j % C::RA) * C::RPC) * TROW;      // row j - RA l + MMIN
-                double wv[P + 2];                                         // compile-time indices only: registers
-#pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    if ((t & 1) == 0 && t <= P) {                         // vertices t, t+1 (column 17 is zero padding)
-                        const double2 w2 = __ldg(src + j * 9 + t / 2);    // warp-uniform address: L1 broadcast
-                        wv[t] = w2.x;
-                        wv[t + 1] = w2.y;
-                    }
-#pragma unroll
-                    for (int cc = 0; cc < NCLS; ++cc) {
-                        const double2 Tv = trow[C::coarser ? F * t - cc : t];
-#pragma unroll
-                        for (int m = 0; m < MT; ++m) {
-                            const int i = C::finer ? t + F * m - F * (kBlkR - 1) : t + m - (MT - 1);    // compile-time
-                            if (i >= 0 && i <= P) {
-                                ax[cc * MT + m] = fma(wv[i], Tv.x, ax[cc * MT + m]);
-                                ay[cc * MT + m] = fma(wv[i], Tv.y, ay[cc * MT + m]);
-                            }
-                        }
-                    }
-                }
-            }
+            correlate_patch<V>(T, src, __ldg(pflags + b), l, h, ax, ay);
         };
         __syncthreads();                                                  // sPos is visible
 
@@ -301,7 +274,7 @@ void launch_lattice_corr_one(const DevLayout &d, const PatchArrays &pa, const La
     const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(2) * sms));
     const double *wq = n_planes == 1 ? pa.wQ : la.wS;
     lattice_corr_kernel<V><<<grid, kOffWarps * 32, LatCls<V>::smem, s>>>(
-        pa.info, pa.levels, groups, pa.pmap, wq, int64_t(pa.n_patches) * kPatchQStride, la.fn, la.meta, n_planes,
+        pa.info, pa.levels, groups, pa.pmap, wq, int64_t(pa.n_patches) * kPatchQStride, pa.pflags, la.fn, la.meta, n_planes,
         n_groups, po.n_split, po.first_patch, po.last_patch, first, count, part, d.queue + 1 + V);
 }
 

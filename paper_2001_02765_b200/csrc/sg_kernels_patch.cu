@@ -225,7 +225,7 @@ patch_far_kernel(const PatchInfo *__restrict__ info, const double *__restrict__ 
 #pragma unroll 4
                 for (int j = 0; j <= P; ++j, v += dv) {
                     const double w = sw[j * (P + 2) + i];
-                    const double q = fma(v, v, uu);
+                    const double q = fmax(fma(v, v, uu), 0.5);        // 0 only for a hole of a padded layout (discarded)
                     const double y0 = rsqrt_approx(q);
                     const double t = q * y0;
                     const double e = fma(-t, y0, 1.0);
@@ -318,7 +318,8 @@ template <int V>
 __global__ void __launch_bounds__(kOffWarps * 32, 2)
 patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__restrict__ levels,
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
-                    const double *__restrict__ wQ, const double *__restrict__ lntab_g, int tab_idx0, int n_groups,
+                    const double *__restrict__ wQ, const int32_t *__restrict__ pflags,
+                    const double *__restrict__ lntab_g, int tab_idx0, int n_groups,
                     int n_split, int first_patch, int last_patch, int64_t first, int64_t count,
                     double *__restrict__ part, unsigned int *__restrict__ queue, uint32_t keep) {
     using C = OffCls<V>;
@@ -327,17 +328,11 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     // per thread and source row: coarser source: NCLS column classes of MT targets each, NT table steps;
     // otherwise 8 consecutive targets, NT table entries
     constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
-    constexpr int NT = C::finer ? P + F * (kBlkR - 1) + 1 : P + MT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2 *sT = reinterpret_cast<double2 *>(smem_raw);                   // [2 or 1][TBUF] offset tables
-    double *sW = reinterpret_cast<double *>(sT + (C::DB ? 2 : 1) * TBUF);  // [warp][17][8 | 18 | 6] weights of B_w
     __shared__ int s_item;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int l = lane & 15, h = lane >> 4;
-
-    if (!C::WG)
-        for (int i = tid; i < kOffWarps * kBlkW; i += kOffWarps * 32) sW[i] = 0.0;       // the padding stays zero
-    double *W = sW + warp * kBlkW;
 
     const int n_items = n_groups * n_split;
     while (true) {
@@ -407,51 +402,8 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                 }
         };
         auto consume = [&](int b, const double2 *T) {
-            // stage the weights of B: global [17][18] (column 17 is zero) -> shared [17][8 | 18 | 6]
-            const double2 *src = reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride);
-            if (!C::WG) {
-                __syncwarp();
-#pragma unroll
-                for (int q = 0; q < 5; ++q) {
-                    const int e2 = lane + 32 * q;
-                    if (e2 < 17 * 9) {
-                        const int j = e2 / 9, c2 = e2 - 9 * j;
-                        *reinterpret_cast<double2 *>(W + j * kBlkWRow + 8 + 2 * c2) = src[e2];
-                    }
-                }
-                __syncwarp();
-            }
-            // entry (row, col) = (j RB - l RA + MMIN, i RB - k RA + MMIN) for vertex (i, j) and target (k, l)
-            if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;   // column F t + this - cc
-            else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
-#pragma unroll 1
-            for (int j = 0; j <= P; ++j) {
-                const double2 *trow = C::coarser ? T + F * j * TROW                                   // row F j - l + 15
-                                                 : T + (j / C::RA + (j % C::RA) * C::RPC) * TROW;      // row j - RA l + MMIN
-                const double *wrow = W + j * kBlkWRow + 8;                // wrow[i] = weight of vertex i
-                double wv[P + 2];                                         // compile-time indices only: registers
-#pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    if ((t & 1) == 0 && t <= P) {                         // vertices t, t+1 (column 17 is zero padding)
-                        const double2 w2 = C::WG ? __ldg(src + j * 9 + t / 2)           // warp-uniform address: L1 broadcast
-                                                 : *reinterpret_cast<const double2 *>(wrow + t);
-                        wv[t] = w2.x;
-                        wv[t + 1] = w2.y;
-                    }
-#pragma unroll
-                    for (int cc = 0; cc < NCLS; ++cc) {
-                        const double2 Tv = trow[C::coarser ? F * t - cc : t];
-#pragma unroll
-                        for (int m = 0; m < MT; ++m) {
-                            const int i = C::finer ? t + F * m - F * (kBlkR - 1) : t + m - (MT - 1);    // compile-time
-                            if (i >= 0 && i <= P) {
-                                ax[cc * MT + m] = fma(wv[i], Tv.x, ax[cc * MT + m]);
-                                ay[cc * MT + m] = fma(wv[i], Tv.y, ay[cc * MT + m]);
-                            }
-                        }
-                    }
-                }
-            }
+            correlate_patch<V>(T, reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride), __ldg(pflags + b), l, h,
+                               ax, ay);
         };
 
         bool any_cur = false, any_next = false;
@@ -516,7 +468,7 @@ void launch_patch_offset_one(const DevLayout &d, const PatchArrays &pa, const Of
     for (int q = 0; q < list; ++q) groups += po.n_groups[q];
     const int grid = int(std::min<int64_t>(int64_t(po.n_split) * n_groups, int64_t(2) * sms));
     patch_offset_kernel<V><<<grid, kOffWarps * 32, OffCls<V>::smem, s>>>(
-        pa.info, pa.levels, groups, pa.pmap, pa.wQ, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,
+        pa.info, pa.levels, groups, pa.pmap, pa.wQ, pa.pflags, d.lntab, d.tab_idx0, n_groups, po.n_split, po.first_patch,
         po.last_patch, first, count, part, d.queue + 1 + V, kLogKeepMask);
 }
 

@@ -52,6 +52,7 @@ struct PatchArrays {
     double *wP = nullptr;             // [n_patches * wstride] per-patch (owned, deduplicated) vertex weights, [j][i]
     int32_t *far_list = nullptr;      // P = 16: per level, the patches >= 3 levels away (patch_far_kernel)
     int32_t *far_meta = nullptr;      // [2 n_levels]: first entry and count of every level's list
+    int32_t *pflags = nullptr;        // [n_patches] bit 0: vertex row P owned somewhere; bit 1: vertex column P (rows < P)
     int32_t *pvmap = nullptr;         // [n_patches * (P+1)^2] global vertex owned by patch vertex (i, j), or -1
 };
 

@@ -105,6 +105,21 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
                 }
         }
     }
+    if (cell_present) {
+        // holes of a padded layout: their results are discarded, but the direct kernels and finalise still run on them.
+        // Give them the position of a real cell (the previous present one, the first for leading holes), so that no hole
+        // can sit on a vertex (r = 0) or outside the range of the log tables; the lattice kernels take target positions
+        // from the patch geometry and do not read these arrays.  The extent below still covers the blocks' full area.
+        for (int64_t c = 0; c < N; ++c) L.extent = std::max(L.extent, std::max(L.tkx[c], L.tky[c]) + 1);
+        int64_t first_present = 0;
+        while (first_present < N && !cell_present[first_present]) ++first_present;
+        if (first_present == N) { err = "no leaf cell present"; return SG_ERR_ARG; }
+        int64_t last = first_present;
+        for (int64_t c = 0; c < N; ++c) {
+            if (cell_present[c]) { last = c; continue; }
+            L.tkx[c] = L.tkx[last]; L.tky[c] = L.tky[last];
+        }
+    }
     L.tX = L.tkx; sorted_unique(L.tX);
     L.tY = L.tky; sorted_unique(L.tY);
     L.itx.resize(N); L.ity.resize(N);

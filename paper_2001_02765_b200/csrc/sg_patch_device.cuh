@@ -23,7 +23,10 @@ __device__ __forceinline__ double fast_ln_g(double a, const double *__restrict__
 
 __device__ __forceinline__ double2 pair_terms_g(double u, double v, const double *__restrict__ lntab_g, int tab_idx0,
                                                 uint32_t keep) {
-    const double q = fma(u, u, v * v);
+    // q >= 1 for every real pair (a target never sits on a vertex).  The clamp only matters for the holes of a padded
+    // layout (regrouped small patches), whose discarded targets may coincide with a vertex: it keeps r finite and the
+    // log-table index in range
+    const double q = fmax(fma(u, u, v * v), 0.5);
     const double y0 = rsqrt_approx(q);
     const double t = q * y0;
     const double e = fma(-t, y0, 1.0);
@@ -46,9 +49,73 @@ struct OffCls {
     static constexpr int TBUF = ROWS * TROW;
     static constexpr bool DB = F < 4;                                     // double-buffered tables (two CTAs per SM)
     static constexpr int LDIST = coarser ? -(F == 2 ? 1 : 2) : finer ? (F == 2 ? 1 : 2) : 0;   // source level - target level
-    static constexpr bool WG = F == 4;                                    // weights straight from global / L1: the table
-                                                                          // leaves no room for weight buffers at 2 CTAs per SM
-    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16 + (WG ? 0 : size_t(kOffWarps) * kBlkW * 8);
+    // weights are read straight from global memory (warp-uniform addresses: an L1 broadcast), shared memory holds tables only
+    static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16;
 };
+
+// Correlation of one target patch (this warp: lane = l + 16 h, l = target row, 8 targets per thread) with the vertices
+// of one source patch through the offset table T of the patch pair; shared by patch_offset_kernel (tables built in the
+// CTA) and lattice_corr_kernel (tables streamed from the function lattices), so that both give bit-identical sums.
+// With vertex (i, j) of B and target (k, l) of A the table entry is T[j rb - l ra + 15 ra][i rb - k ra + 15 ra]:
+//   same level (ra = rb = 1): thread owns columns k = 8 h + r; entry column t + 8 - 8 h serves vertices i = t + r - 7;
+//   coarser source (ra = 1, rb = F): NCLS = F / 2 column classes mod F of MT = 8 / NCLS targets, k = F m + NCLS h + cc;
+//          entry column F t + F (1 - MT) + 15 - NCLS h - cc serves i = t + m - (MT - 1);
+//   finer source (ra = F, rb = 1): k = 8 h + r; entry column t + 8 F (1 - h) serves i = t + F r - 7 F; table rows are
+//          stored by row class (row j - F l + 15 F has the residue of j mod F: a half-warp reads consecutive stored rows).
+// One loaded entry serves up to 8 targets (16 DFMA per LDS.128); the weights of a source row sit in registers (fully
+// unrolled, compile-time indices, ragged ends removed at compile time).  src: the patch's weights, [17] rows of 9
+// double2 (vertices 2c, 2c+1; vertex 17 is zero padding).  flags (warp-uniform): bit 0 = vertex row 16 of the source
+// patch carries owned vertices, bit 1 = vertex column 16 does (in a row below 16): on a uniform level a patch owns only
+// its 16 x 16 lower-left vertices (sg_api.cu, owner rule), so row 16 and column 16 are skipped for almost every patch --
+// 256 instead of 289 vertices.  Every per-patch sum stays in one accumulator chain.
+template <int V>
+__device__ __forceinline__ void correlate_patch(const double2 *__restrict__ T, const double2 *__restrict__ src, int flags,
+                                                int l, int h, double (&ax)[kBlkR], double (&ay)[kBlkR]) {
+    using C = OffCls<V>;
+    constexpr int P = 16, F = C::F, TROW = C::TROW;
+    constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
+    constexpr int NT = C::finer ? P + F * (kBlkR - 1) : P + MT - 1;       // table steps that reach vertices 0 .. P-1
+    if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;  // column F t + this - cc
+    else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
+    const int jmax = (flags & 1) ? P : P - 1;
+#pragma unroll 1
+    for (int j = 0; j <= jmax; ++j) {
+        const double2 *trow = C::coarser ? T + F * j * TROW                                   // row F j - l + 15
+                                         : T + (j / C::RA + (j % C::RA) * C::RPC) * TROW;      // row j - RA l + MMIN
+        double wv[P];                                                     // compile-time indices only: registers
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            if ((t & 1) == 0 && t < P) {                                  // vertices t, t+1
+                const double2 w2 = __ldg(src + j * 9 + t / 2);            // warp-uniform address: L1 broadcast
+                wv[t] = w2.x;
+                wv[t + 1] = w2.y;
+            }
+#pragma unroll
+            for (int cc = 0; cc < NCLS; ++cc) {
+                const double2 Tv = trow[C::coarser ? F * t - cc : t];
+#pragma unroll
+                for (int m = 0; m < MT; ++m) {
+                    const int i = C::finer ? t + F * m - F * (kBlkR - 1) : t + m - (MT - 1);    // compile-time
+                    if (i >= 0 && i < P) {
+                        ax[cc * MT + m] = fma(wv[i], Tv.x, ax[cc * MT + m]);
+                        ay[cc * MT + m] = fma(wv[i], Tv.y, ay[cc * MT + m]);
+                    }
+                }
+            }
+        }
+        if ((flags & 2) || j == P) {                                      // vertex column 16 of this row
+            const double w16 = __ldg(src + j * 9 + 8).x;
+#pragma unroll
+            for (int cc = 0; cc < NCLS; ++cc)
+#pragma unroll
+                for (int m = 0; m < MT; ++m) {
+                    const int t = C::finer ? P - F * m + F * (kBlkR - 1) : P - m + (MT - 1);   // the step with i(t, m) = 16
+                    const double2 Tv = trow[C::coarser ? F * t - cc : t];
+                    ax[cc * MT + m] = fma(w16, Tv.x, ax[cc * MT + m]);
+                    ay[cc * MT + m] = fma(w16, Tv.y, ay[cc * MT + m]);
+                }
+        }
+    }
+}
 
 }  // namespace sg

