@@ -269,9 +269,9 @@ def run_ours(args):
     exp = expected_counts(args.config)
     assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"], "frozen layout changed"
     N = lay.n_cells
-    lattice = (not args.slopes) and args.mode != "direct" and lay.P in (8, 16)
+    lattice = args.mode != "direct" and (lay.P == 16 or (lay.P == 8 and not args.slopes))
     if args.mode == "lattice" and not lattice:
-        raise SystemExit("--mode lattice needs the zeroth-order path and 8x8 or 16x16 patches")
+        raise SystemExit("--mode lattice needs 16x16 patches (8x8 for the zeroth-order path only)")
     if lattice:
         # lattice mode works on whole patches and a target's cost depends on its level: split by estimated cost
         first, count = shard_range_by_cost(lattice_patch_costs(lay.patches[:, 0]), lay.P * lay.P, rank, world)
@@ -403,15 +403,19 @@ def run_ours(args):
                 "pair_evaluations_per_launch": evals,
             }
 
-        direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
-        direct_traffic = measured_traffic(workload_name(args.config), direct_name) if world == 1 else None
         if args.slopes:
-            roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, "interaction_lin_kernel<4>",
-                                   measured_traffic(workload_name(args.config), "interaction_lin_kernel<4>") if world == 1 else None)
-        elif lattice:
-            lattice_name = "patch_offset_kernel<0> (same-level pairs; <1>..<4> for pairs one and two levels apart)"
+            direct_name = "interaction_lin_kernel<4>"
+        else:
+            direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
+        direct_traffic = measured_traffic(workload_name(args.config), direct_name) if world == 1 else None
+        if lattice:
+            lattice_name = ("lattice_corr_kernel<0> (same-level pairs; <1>..<4> for pairs one and two levels apart"
+                            + ("; three planes per offset: slope terms)" if args.slopes else ")"))
+            if lay.P == 8:
+                lattice_name = "patch_interaction_kernel<8>"
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, lattice_name,
-                                   measured_traffic(workload_name(args.config), lattice_name) if world == 1 else None)
+                                   measured_traffic(workload_name(args.config) + ("+slopes" if args.slopes else ""),
+                                                    lattice_name) if world == 1 else None)
         else:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, direct_name, direct_traffic)
         line = {
@@ -421,7 +425,9 @@ def run_ours(args):
             "config": {"workload": workload_name(args.config), "n_cells": N, "n_vertices": info["n_vertices"],
                        "pairs_per_evaluation": pairs,
                        "order": "sigma0 + slope terms (Eq. 6)" if args.slopes else "sigma0 (north_star hot path)",
-                       "interaction_mode": "lattice-offset reuse (SG_MODE_LATTICE)" if lattice else "direct",
+                       "interaction_mode": ("lattice-offset reuse (SG_MODE_LATTICE): precomputed function lattices "
+                                            "streamed by TMA, 2 DFMA per pair" + (" and plane (6 with slopes)" if args.slopes else ""))
+                                           if lattice else "direct",
                        "parallelism": f"targets sharded over {world} GPU(s)" + (" by estimated cost, whole patches" if lattice else " by count"),
                        "create_ms": create_ms,
                        "l2": "256 MiB memset between steps (inside the timed region)"},
@@ -435,7 +441,8 @@ def run_ours(args):
             d_k = sum(d_kms) / max(1, len(d_kms))
             line["direct_kernel"] = {
                 "what": "same workload, same run, SG_MODE_DIRECT: every (target, vertex) pair = 1 sqrt + 2 ln "
-                        f"(the north_star interaction kernel); {DIRECT_LEG_STEPS} timed steps after 3 warm-ups",
+                        f"(the north_star interaction kernel{'; with slope terms' if args.slopes else ''}); "
+                        f"{DIRECT_LEG_STEPS} timed steps after 3 warm-ups",
                 "value": pairs * DIRECT_LEG_STEPS / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / DIRECT_LEG_STEPS,
                 "steps": DIRECT_LEG_STEPS, "warmup": 3,
                 "roofline": roofline_of(d_model, d_k, d_total / DIRECT_LEG_STEPS, direct_name, direct_traffic)}

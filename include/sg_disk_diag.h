@@ -27,6 +27,15 @@ extern "C" {
  */
 int sg_lattice_plan_check(const sg_ctx *ctx, int64_t *out);
 
+/*
+ * Fill of the offset walk (P = 16), host only: per pair class V, out[3 V] = offsets visited by all target groups,
+ * out[3 V + 1] = offsets at which at least one of the group's <= 8 target patches has a source patch (one table each),
+ * out[3 V + 2] = patch pairs.  pairs / (8 * live offsets) is the fraction of warp slots with work when the warps of a
+ * CTA move through the offsets in lock step (patch_offset_kernel); lattice_corr_kernel lets them drift apart by the
+ * depth of its stage ring (profiles/r2_*).  out: host [15].
+ */
+int sg_lattice_plan_fill(const sg_ctx *ctx, int64_t *out);
+
 /* Number of kernel launches one sg_set_density / one sg_force enqueues with the current settings. */
 int sg_launch_counts(const sg_ctx *ctx, int *set_density_launches, int *force_launches);
 

@@ -20,7 +20,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 # every symbol include/sg_disk.h and include/sg_disk_diag.h declare (tests check the headers and this list agree)
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
-    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
+    "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_lattice_plan_fill", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_kernel_instruction_counts", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
 )
 
@@ -79,6 +79,8 @@ def load_library():
     lib.sg_set_interaction_mode.argtypes = [vp, c_int]
     lib.sg_lattice_plan_check.restype = c_int
     lib.sg_lattice_plan_check.argtypes = [vp, ctypes.POINTER(c_i64)]
+    lib.sg_lattice_plan_fill.restype = c_int
+    lib.sg_lattice_plan_fill.argtypes = [vp, ctypes.POINTER(c_i64)]
     lib.sg_launch_counts.restype = c_int
     lib.sg_launch_counts.argtypes = [vp, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
     lib.sg_set_kernel_timing.restype = c_int
@@ -226,6 +228,13 @@ class SgDisk:
         v = list(out)
         return {"pairs_per_class": v[0:5], "duplicates": v[5], "wrong_level": v[6], "groups": v[7:10],
                 "offsets": v[10], "available": bool(v[11]), "patches_missing_from_launched_lists": v[12]}
+
+    def lattice_plan_fill(self):
+        """Per pair class: offsets visited, offsets with a source patch for some target of the group, patch pairs."""
+        out = (ctypes.c_int64 * 15)()
+        self._check(self._lib.sg_lattice_plan_fill(self._ctx, out))
+        v = list(out)
+        return [dict(offsets=v[3 * k], live_offsets=v[3 * k + 1], pairs=v[3 * k + 2]) for k in range(5)]
 
     def force(self, Fx=None, Fy=None):
         """Fx, Fy (CUDA float64 [count]) at the leaf centres of the current target range."""

@@ -1038,6 +1038,45 @@ int sg_lattice_plan_check(const sg_ctx *c, int64_t *out) {
     return SG_OK;
 }
 
+int sg_lattice_plan_fill(const sg_ctx *c, int64_t *out) {
+    if (!c || !out) return SG_ERR_ARG;
+    for (int i = 0; i < 3 * kOffClasses; ++i) out[i] = 0;
+    if (!c->patch_plan_ok) return SG_OK;
+    const HostLayout &h = c->host;
+    const int F_of[kOffClasses] = {1, 2, 2, 4, 4}, dl_of[kOffClasses] = {0, -1, 1, -2, 2};
+    size_t g0 = 0;
+    for (int list = 0; list < 3; ++list) {
+        for (size_t gi = g0; gi < g0 + size_t(c->patch_n_groups[list]); ++gi) {
+            const PatchGroup &g = c->patch_groups[gi];
+            for (int v = 0; v < kOffClasses; ++v) {
+                if (offset_group_list(v) != list) continue;
+                const int ndpi = g.box[v][1], ndpj = g.box[v][3];
+                if (ndpi * ndpj == 0) continue;
+                const int F = F_of[v], step = dl_of[v] < 0 ? F : 1;
+                const PatchLevel &slev = c->patch_levels[size_t(g.level + dl_of[v])];
+                for (int n = 0; n < ndpi * ndpj; ++n) {
+                    int hits = 0;
+                    for (int w = 0; w < g.n; ++w) {
+                        const int api = h.patches[size_t(g.patch[w])].i0 / h.P, apj = h.patches[size_t(g.patch[w])].j0 / h.P;
+                        const int dx = g.box[v][0] + step * (n % ndpi), dy = g.box[v][2] + step * (n / ndpi);
+                        int bi, bj;
+                        if (dl_of[v] < 0) { bi = (api + dx) / F; bj = (apj + dy) / F; }
+                        else { bi = F * api + dx; bj = F * apj + dy; }
+                        bi -= slev.pimin; bj -= slev.pjmin;
+                        if (bi < 0 || bi >= slev.npx || bj < 0 || bj >= slev.npy) continue;
+                        hits += c->patch_pmap[size_t(slev.map_off) + size_t(bj) * slev.npx + bi] >= 0;
+                    }
+                    out[3 * v] += 1;
+                    out[3 * v + 1] += hits > 0;
+                    out[3 * v + 2] += hits;
+                }
+            }
+        }
+        g0 += size_t(c->patch_n_groups[list]);
+    }
+    return SG_OK;
+}
+
 int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     if (!c) return SG_ERR_ARG;
     if (c->inner) {                                               // + the permutation kernels

@@ -84,12 +84,22 @@ constexpr int kLatAuxBytes = kChunkOffsets * 8 * 4      // sB: source patch of (
 // dynamic shared memory per CTA with two CTAs per SM: (228 KB - 2 x 1 KB reserved) / 2, minus a little static room
 constexpr int kLatSmemBudget = 115712 - 256;
 
+// A stage of the ring holds a whole table (classes at most one level apart) or a SUB-BLOCK of its rows: the 80-row
+// tables of the classes two levels apart (104 KB) would leave room for one stage only, i.e. lock step.
+//   source two levels coarser (V = 3): source row j needs table rows 4 j .. 4 j + 15; sub-block s = the rows of source
+//       rows 4 s .. 4 s + 3 = table rows 16 s .. 16 s + 27 (s = 4: row 16 only, table rows 64 .. 79); 5 sub-blocks that
+//       overlap by 12 rows (the rows are fetched twice; TMA traffic is not the bottleneck)
+//   source two levels finer (V = 4): the table is stored by residue class of the source row (j mod 4), and the source
+//       rows are correlated class by class (OffCls::JPASSES): sub-block c = the 20 stored rows of class c
 template <int V>
 struct LatCls {
     using C = OffCls<V>;
-    static constexpr int STAGE_BYTES = C::TBUF * 16;
+    static constexpr int NSUB = V == kOffCoarserSrc4 ? 5 : V == kOffFinerSrc4 ? 4 : 1;
+    static constexpr int SLOT_ROWS = V == kOffCoarserSrc4 ? 28 : V == kOffFinerSrc4 ? C::RPC : C::ROWS;
+    static constexpr int SLOT_ENTRIES = SLOT_ROWS * C::TROW;
+    static constexpr int STAGE_BYTES = SLOT_ENTRIES * 16;
     static constexpr int K_FIT = (kLatSmemBudget - kLatAuxBytes) / STAGE_BYTES;
-    static constexpr int K = K_FIT < 1 ? 1 : (K_FIT > 6 ? 6 : K_FIT);        // ring depth: 6, 3, 3, 1, 1
+    static constexpr int K = K_FIT < 1 ? 1 : (K_FIT > 6 ? 6 : K_FIT);        // ring depth: 6, 3, 3, 3, 4
     static constexpr size_t smem = size_t(K) * STAGE_BYTES + kLatAuxBytes;
 };
 
@@ -103,7 +113,8 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                     int last_patch, int64_t first, int64_t count, double *__restrict__ part,
                     unsigned int *__restrict__ queue) {
     using C = OffCls<V>;
-    constexpr int P = 16, F = C::F, TROW = C::TROW, TBUF = C::TBUF, K = LatCls<V>::K;
+    constexpr int P = 16, F = C::F, TROW = C::TROW, TBUF = LatCls<V>::SLOT_ENTRIES, K = LatCls<V>::K;
+    constexpr int NSUB = LatCls<V>::NSUB;
     constexpr int STEP = C::coarser ? F : 1;                              // offsets keep A + d a multiple of F
     constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -150,26 +161,37 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
 #pragma unroll
         for (int r = 0; r < kBlkR; ++r) { ax[r] = 0.0; ay[r] = 0.0; }
 
-        // the copies of stage s of the current chunk (offset sLive[s / n_planes], plane s % n_planes), by one warp
+        // the copies of stage s of the current chunk: stage = (live offset m, plane pl, sub-block sub), by one warp
         auto issue_stage = [&](int s, int cb) {
-            const int m = n_planes == 1 ? s : s / n_planes, pl = s - m * n_planes;
+            const int sub = NSUB == 1 ? 0 : s % NSUB, sp2 = NSUB == 1 ? s : s / NSUB;
+            const int m = n_planes == 1 ? sp2 : sp2 / n_planes, pl = sp2 - m * n_planes;
             const int n = cb + sLive[m];
             const int dx = dpi_min + STEP * (n % ndpi), dy = dpj_min + STEP * (n / ndpi);
             const double2 *src = fn + fm.base + int64_t(pl) * fm.plane_stride +
                                  int64_t(P * dy - fm.rmin) * fm.ncols + (P * dx - fm.cmin);
             const uint32_t slot = (gs + uint32_t(s)) % K;
-            if (lane == 0) mbar_expect_tx(&full[slot], C::ROWS * TROW * 16);
+            const int nrows = V == kOffCoarserSrc4 ? (sub < 4 ? 28 : 16) : LatCls<V>::SLOT_ROWS;
+            if (lane == 0) mbar_expect_tx(&full[slot], uint32_t(nrows) * TROW * 16);
             __syncwarp();
-            for (int pos = lane; pos < C::ROWS; pos += 32) {
-                const int nn = (pos % C::RPC) * C::RA + pos / C::RPC;       // stored row pos holds table row nn
-                tma_bulk_g2s(ring + slot * TBUF + pos * TROW, src + int64_t(nn) * fm.ncols, TROW * 16, &full[slot]);
+            for (int r = lane; r < nrows; r += 32) {
+                // table row held by slot row r
+                const int nn = V == kOffCoarserSrc4 ? 16 * sub + r
+                             : V == kOffFinerSrc4   ? r * C::RA + sub
+                                                    : (r % C::RPC) * C::RA + r / C::RPC;
+                tma_bulk_g2s(ring + slot * TBUF + r * TROW, src + int64_t(nn) * fm.ncols, TROW * 16, &full[slot]);
             }
         };
         // correlation of target patch `my_patch` with the vertices of source patch b (weights of plane pl) through
         // the table T: correlate_patch, shared with patch_offset_kernel
-        auto consume = [&](int b, int pl, const double2 *T) {
+        auto consume = [&](int b, int pl, int sub, const double2 *T) {
             const double2 *src = reinterpret_cast<const double2 *>(wq + int64_t(pl) * w_plane_stride + int64_t(b) * kPatchQStride);
-            correlate_patch<V>(T, src, __ldg(pflags + b), l, h, ax, ay);
+            const int flags = __ldg(pflags + b);
+            if (V == kOffCoarserSrc4)            // slot row 0 = table row 16 sub; source rows 4 sub .. 4 sub + 3
+                correlate_patch<V>(T - 16 * sub * TROW, src, flags, l, h, ax, ay, 4 * sub, min(4 * sub + 3, P), 1);
+            else if (V == kOffFinerSrc4)         // slot row 0 = stored row sub RPC; source rows sub, sub + 4, ...
+                correlate_patch<V>(T - sub * C::RPC * TROW, src, flags, l, h, ax, ay, sub, P, 4);
+            else
+                correlate_patch<V>(T, src, flags, l, h, ax, ay, 0, P, 1);
         };
         __syncthreads();                                                  // sPos is visible
 
@@ -207,16 +229,17 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                 if (lane == 0) sMisc[1] = cnt;
             }
             __syncthreads();
-            const int S = sMisc[1] * n_planes;                            // stages of this chunk
+            const int S = sMisc[1] * n_planes * NSUB;                     // stages of this chunk
             // (3) the ring: warp 0 fills the first K stages, afterwards the last warp to release a stage refills it
             if (warp == 0)
                 for (int s = 0; s < min(K, S); ++s) issue_stage(s, cb);
             for (int s = 0; s < S; ++s) {
-                const int m = n_planes == 1 ? s : s / n_planes, pl = s - m * n_planes;
+                const int sub = NSUB == 1 ? 0 : s % NSUB, sp2 = NSUB == 1 ? s : s / NSUB;
+                const int m = n_planes == 1 ? sp2 : sp2 / n_planes, pl = sp2 - m * n_planes;
                 const int b = sB[sLive[m] * 8 + warp];
                 const uint32_t g = gs + uint32_t(s), slot = g % K;
                 mbar_wait(&full[slot], (g / K) & 1u);                     // also for a warp without work: a warp
-                if (my_patch >= 0 && b >= 0) consume(b, pl, ring + slot * TBUF);   // never runs more than K stages ahead
+                if (my_patch >= 0 && b >= 0) consume(b, pl, sub, ring + slot * TBUF);   // never runs more than K stages ahead
                 __syncwarp();
                 int last = 0;
                 if (lane == 0) {

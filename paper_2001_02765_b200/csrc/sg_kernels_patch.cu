@@ -402,8 +402,8 @@ patch_offset_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                 }
         };
         auto consume = [&](int b, const double2 *T) {
-            correlate_patch<V>(T, reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride), __ldg(pflags + b), l, h,
-                               ax, ay);
+            correlate_patch_all<V>(T, reinterpret_cast<const double2 *>(wQ + int64_t(b) * kPatchQStride), __ldg(pflags + b),
+                                   l, h, ax, ay);
         };
 
         bool any_cur = false, any_next = false;

@@ -51,6 +51,10 @@ struct OffCls {
     static constexpr int LDIST = coarser ? -(F == 2 ? 1 : 2) : finer ? (F == 2 ? 1 : 2) : 0;   // source level - target level
     // weights are read straight from global memory (warp-uniform addresses: an L1 broadcast), shared memory holds tables only
     static constexpr size_t smem = size_t(DB ? 2 : 1) * TBUF * 16;
+    // Order in which the source rows of a patch are correlated: natural, except for the source two levels finer, whose
+    // table rows are stored by residue class of j mod 4 -- there class by class (j = c, c + 4, ...), so that one class
+    // block of the table is needed at a time (lattice_corr_kernel streams it in four sub-blocks).
+    static constexpr int JPASSES = V == kOffFinerSrc4 ? 4 : 1;
 };
 
 // Correlation of one target patch (this warp: lane = l + 16 h, l = target row, 8 targets per thread) with the vertices
@@ -68,18 +72,21 @@ struct OffCls {
 // patch carries owned vertices, bit 1 = vertex column 16 does (in a row below 16): on a uniform level a patch owns only
 // its 16 x 16 lower-left vertices (sg_api.cu, owner rule), so row 16 and column 16 are skipped for almost every patch --
 // 256 instead of 289 vertices.  Every per-patch sum stays in one accumulator chain.
+// Source rows j0, j0 + jstep, ... <= j1 only (the whole patch: 0, 16, 1): lattice_corr_kernel streams the large
+// tables of the classes two levels apart in sub-blocks of rows and correlates the source rows of one sub-block at a time.
 template <int V>
 __device__ __forceinline__ void correlate_patch(const double2 *__restrict__ T, const double2 *__restrict__ src, int flags,
-                                                int l, int h, double (&ax)[kBlkR], double (&ay)[kBlkR]) {
+                                                int l, int h, double (&ax)[kBlkR], double (&ay)[kBlkR], int j0, int j1,
+                                                int jstep) {
     using C = OffCls<V>;
     constexpr int P = 16, F = C::F, TROW = C::TROW;
     constexpr int NCLS = C::coarser ? F / 2 : 1, MT = kBlkR / NCLS;
     constexpr int NT = C::finer ? P + F * (kBlkR - 1) : P + MT - 1;       // table steps that reach vertices 0 .. P-1
     if (C::coarser) T += (15 - l) * TROW + F * (1 - MT) + 15 - NCLS * h;  // column F t + this - cc
     else T += (15 - l) * TROW + 8 * F * (1 - h);                          // column t + this (F = 1: 8 - 8 h)
-    const int jmax = (flags & 1) ? P : P - 1;
+    const int jmax = min(j1, (flags & 1) ? P : P - 1);
 #pragma unroll 1
-    for (int j = 0; j <= jmax; ++j) {
+    for (int j = j0; j <= jmax; j += jstep) {
         const double2 *trow = C::coarser ? T + F * j * TROW                                   // row F j - l + 15
                                          : T + (j / C::RA + (j % C::RA) * C::RPC) * TROW;      // row j - RA l + MMIN
         double wv[P];                                                     // compile-time indices only: registers
@@ -117,5 +124,14 @@ __device__ __forceinline__ void correlate_patch(const double2 *__restrict__ T, c
         }
     }
 }
+
+// the whole source patch, in the row order of the class (both kernel families: bit-identical sums)
+template <int V>
+__device__ __forceinline__ void correlate_patch_all(const double2 *__restrict__ T, const double2 *__restrict__ src,
+                                                    int flags, int l, int h, double (&ax)[kBlkR], double (&ay)[kBlkR]) {
+#pragma unroll 1
+    for (int c = 0; c < OffCls<V>::JPASSES; ++c) correlate_patch<V>(T, src, flags, l, h, ax, ay, c, 16, OffCls<V>::JPASSES);
+}
+
 
 }  // namespace sg

@@ -218,3 +218,19 @@ def test_bench_gpus_n_spawns_n_ranks():
         del os.environ["WORLD_SIZE"]
     assert bench.spawn_command(type("A", (), {"impl": "ours", "gpus": 1})(), []) is None
     assert bench.spawn_command(type("A", (), {"impl": "reference", "gpus": 4})(), []) is None
+
+
+def test_lattice_plan_fill_of_the_amr_configs():
+    """The numbers profiles/r2_captureA quotes for the lock-step fill of the offset walk (host replay): pairs per class
+    equal the level-count products, and on cfg 4 only 61 % (same level) / 28-36 % (cross level) of the warp slots of a
+    lock-step CTA have work, against 94 % on the uniform cfg 5."""
+    lay, _ = make_config(4)
+    with SgDisk.from_layout(lay, device=-1) as d:
+        fill = d.lattice_plan_fill()
+    assert [f["pairs"] for f in fill] == _near_pair_counts(lay)
+    frac = [f["pairs"] / (8.0 * f["live_offsets"]) for f in fill]
+    assert [round(x, 2) for x in frac] == [0.61, 0.32, 0.36, 0.32, 0.28]
+    lay5, _ = make_config(5)
+    with SgDisk.from_layout(lay5, device=-1) as d:
+        f5 = d.lattice_plan_fill()[0]
+    assert f5["pairs"] == 4096 * 4096 and round(f5["pairs"] / (8.0 * f5["live_offsets"]), 2) == 0.94
