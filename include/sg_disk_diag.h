@@ -74,6 +74,11 @@ int sg_kernel_instruction_counts(int kernel, double *fp64_instr_per_pair, double
  * in FP64 TFLOP/s (FMA = 2), and the same as warp-instructions/s.  Synchronous. */
 int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s);
 
+/* Diagnostic: FP64 tensor-core rate (mma.sync.m8n8k4.f64, 512 flop per warp instruction) alone, and the total rate
+ * of a loop that interleaves one DFMA with every DMMA: if the two shared nothing the second would be the sum of the
+ * DMMA and DFMA peaks (DESIGN.md 6b uses this to decide against a tensor-core formulation).  Synchronous. */
+int sg_measure_fp64_mma_peak(int device, double *dmma_tflops, double *mixed_tflops);
+
 #ifdef __cplusplus
 }
 #endif

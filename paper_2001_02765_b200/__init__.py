@@ -4,5 +4,5 @@ Thin ctypes binding over the C ABI of include/sg_disk.h (argument marshalling on
 the path runs in the CUDA kernels of csrc/).  There is no CPU fallback: if libsg_disk.so is missing
 the import of :mod:`.binding` fails loudly.
 """
-from .binding import (SgDisk, SgError, lib_path, load_library, measure_fp64_peak, version,  # noqa: F401
+from .binding import (SgDisk, SgError, lib_path, load_library, measure_fp64_peak, measure_fp64_mma_peak, version,  # noqa: F401
                       shard_range, EXPORTED_SYMBOLS)

@@ -21,7 +21,7 @@ _ERR_NAMES = {SG_ERR_ARG: "SG_ERR_ARG", SG_ERR_LAYOUT: "SG_ERR_LAYOUT", SG_ERR_C
 EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
     "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_lattice_plan_fill", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
-    "sg_kernel_model", "sg_kernel_instruction_counts", "sg_measure_fp64_peak", "sg_last_error", "sg_version",
+    "sg_kernel_model", "sg_kernel_instruction_counts", "sg_measure_fp64_peak", "sg_measure_fp64_mma_peak", "sg_last_error", "sg_version",
 )
 
 
@@ -93,6 +93,8 @@ def load_library():
     lib.sg_kernel_instruction_counts.argtypes = [c_int, dp, dp]
     lib.sg_measure_fp64_peak.restype = c_int
     lib.sg_measure_fp64_peak.argtypes = [c_int, dp, dp]
+    lib.sg_measure_fp64_mma_peak.restype = c_int
+    lib.sg_measure_fp64_mma_peak.argtypes = [c_int, dp, dp]
     lib.sg_last_error.restype = ctypes.c_char_p
     lib.sg_last_error.argtypes = [vp]
     lib.sg_version.restype = ctypes.c_char_p
@@ -123,6 +125,16 @@ def measure_fp64_peak(device: int = 0):
     if rc != SG_OK:
         raise SgError(rc, lib.sg_last_error(None).decode())
     return tf.value, wi.value
+
+
+def measure_fp64_mma_peak(device: int = 0):
+    """(FP64 TFLOP/s of mma.sync.m8n8k4.f64 alone, total TFLOP/s of DMMA interleaved 1:1 with DFMA)."""
+    lib = load_library()
+    a, b = ctypes.c_double(), ctypes.c_double()
+    rc = lib.sg_measure_fp64_mma_peak(int(device), ctypes.byref(a), ctypes.byref(b))
+    if rc != SG_OK:
+        raise SgError(rc, lib.sg_last_error(None).decode())
+    return a.value, b.value
 
 
 from .sharding import shard_range  # noqa: E402,F401  (re-exported: one definition of the partition)

@@ -500,12 +500,18 @@ int upload_patches(sg_ctx *c) {
         };
         std::vector<int32_t> pv(size_t(pa.n_patches) * P1 * P1, -1), owner(size_t(h.Nv), -1);
         std::vector<int8_t> owner_rank(size_t(h.Nv), 127);
+#pragma omp parallel for schedule(static)
+        for (int p = 0; p < pa.n_patches; ++p) {                   // the look-ups (read only), in parallel
+            const PatchInfo &q = c->patch_info[size_t(p)];
+            for (int j = 0; j < P1; ++j)
+                for (int i = 0; i < P1; ++i)
+                    pv[(size_t(p) * P1 + j) * P1 + i] = vertex_of(q.X0 + i * q.cw, q.Y0 + j * q.cw);
+        }
         for (int p = 0; p < pa.n_patches; ++p) {
             const PatchInfo &q = c->patch_info[size_t(p)];
             for (int j = 0; j < P1; ++j)
                 for (int i = 0; i < P1; ++i) {
-                    const int32_t v = vertex_of(q.X0 + i * q.cw, q.Y0 + j * q.cw);
-                    pv[(size_t(p) * P1 + j) * P1 + i] = v;
+                    const int32_t v = pv[(size_t(p) * P1 + j) * P1 + i];
                     if (v < 0) continue;                           // a lattice point of a padded block that no cell touches
                     const int8_t rank = int8_t((j == h.P ? 2 : 0) + (i == h.P ? 1 : 0));
                     int32_t &o = owner[size_t(v)];
@@ -1189,6 +1195,14 @@ int sg_measure_fp64_peak(int device, double *tflops, double *warp_instr_per_s) {
     cudaError_t e = guard.err;
     if (e == cudaSuccess) e = measure_dfma(tflops, warp_instr_per_s);
     if (e != cudaSuccess) { g_create_error = std::string("sg_measure_fp64_peak: ") + cudaGetErrorString(e); return SG_ERR_CUDA; }
+    return SG_OK;
+}
+
+int sg_measure_fp64_mma_peak(int device, double *dmma_tflops, double *mixed_tflops) {
+    DeviceGuard guard(device);
+    cudaError_t e = guard.err;
+    if (e == cudaSuccess) e = measure_dmma(dmma_tflops, mixed_tflops);
+    if (e != cudaSuccess) { g_create_error = std::string("sg_measure_fp64_mma_peak: ") + cudaGetErrorString(e); return SG_ERR_CUDA; }
     return SG_OK;
 }
 

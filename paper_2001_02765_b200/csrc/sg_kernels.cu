@@ -424,4 +424,67 @@ cudaError_t measure_dfma(double *tflops, double *warp_instr_per_s) {
     return cudaSuccess;
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// FP64 tensor-core probe ("FP64 tensor cores do not help").  mma.sync.m8n8k4.f64 = 512 flop per warp
+// instruction, four independent accumulator pairs per thread; MIX adds four independent DFMA chains per thread in
+// the same loop (one DFMA per DMMA), to see whether the two add up or share one pipe.
+// ------------------------------------------------------------------------------------------------
+template <bool MIX>
+__global__ void __launch_bounds__(256) dmma_kernel(double *out, int iters, double a, double b) {
+    double c[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3;
+    const double fa = a + 1e-9 * threadIdx.x, fb = b;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                             : "+d"(c[q][0]), "+d"(c[q][1]) : "d"(fa), "d"(fb));
+            if (MIX) { x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b); }
+        }
+    }
+    const double sum = c[0][0] + c[0][1] + c[1][0] + c[1][1] + c[2][0] + c[2][1] + c[3][0] + c[3][1] + x0 + x1 + x2 + x3;
+    if (sum == 123.456) out[0] = sum;   // never true; keeps the chains alive
+}
+
+cudaError_t measure_dmma(double *dmma_tflops, double *mixed_tflops) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    double *out = nullptr;
+    e = cudaMalloc(&out, 8);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int grid = sms * 4, iters = 2048;
+    double res[2] = {0.0, 0.0};
+    for (int mix = 0; mix < 2 && e == cudaSuccess; ++mix) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {
+            cudaEventRecord(e0);
+            if (mix) dmma_kernel<true><<<grid, 256>>>(out, iters, 0.999999, 1e-9);
+            else dmma_kernel<false><<<grid, 256>>>(out, iters, 0.999999, 1e-9);
+            cudaEventRecord(e1);
+            e = cudaEventSynchronize(e1);
+            if (e != cudaSuccess) break;
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        const double warps = double(grid) * 8.0, steps = double(iters) * 4.0;
+        const double flop = warps * steps * (4.0 * 512.0 + (mix ? 4.0 * 32.0 * 2.0 : 0.0));   // per warp and step
+        res[mix] = flop / (best * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    if (e != cudaSuccess) return e;
+    if (dmma_tflops) *dmma_tflops = res[0];
+    if (mixed_tflops) *mixed_tflops = res[1];
+    return cudaSuccess;
+}
+
 }  // namespace sg

@@ -93,6 +93,7 @@ void launch_line_tables(const DevLayout &d, cudaStream_t s);
 void launch_interaction(const DevLayout &d, const ForcePlan &p, cudaStream_t s);
 void launch_finalise(const DevLayout &d, const ForcePlan &p, double *Fx, double *Fy, cudaStream_t s);
 cudaError_t measure_dfma(double *tflops, double *warp_instr_per_s);
+cudaError_t measure_dmma(double *dmma_tflops, double *mixed_tflops);   // FP64 mma.sync alone / interleaved with DFMA
 // regrouped layouts: caller cell order <-> padded block order (b, c may be null: sigma only)
 void launch_scatter_cells(const double *a, const double *b, const double *c, const int32_t *inv, double *oa, double *ob,
                           double *oc, int64_t n_inner, cudaStream_t s);

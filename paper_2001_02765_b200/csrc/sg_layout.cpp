@@ -6,8 +6,13 @@
 
 #include <algorithm>
 #include <cmath>
+#include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <unordered_set>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace sg {
 namespace {
@@ -22,8 +27,31 @@ std::string fmt(const char *f, long long a = 0, long long b = 0, long long c = 0
     return buf;
 }
 
+// std::sort over chunks in parallel, then pairwise merges (the layout build is host work a regridding caller pays at
+// every regrid: PAPER.md:265; the 4N-record sort was most of it)
+template <class It, class Cmp>
+void parallel_sort(It first, It last, Cmp cmp) {
+    const int64_t n = last - first;
+    int nt = 1;
+#ifdef _OPENMP
+    nt = std::max(1, std::min(omp_get_max_threads(), 32));
+#endif
+    if (n < (int64_t(1) << 16) || nt == 1) { std::sort(first, last, cmp); return; }
+    int chunks = 1;
+    while (chunks * 2 <= nt) chunks *= 2;
+    std::vector<int64_t> cut(size_t(chunks) + 1);
+    for (int c = 0; c <= chunks; ++c) cut[size_t(c)] = n * c / chunks;
+#pragma omp parallel for schedule(static, 1)
+    for (int c = 0; c < chunks; ++c) std::sort(first + cut[size_t(c)], first + cut[size_t(c) + 1], cmp);
+    for (int width = 1; width < chunks; width *= 2) {
+#pragma omp parallel for schedule(static, 1)
+        for (int c = 0; c < chunks; c += 2 * width)
+            std::inplace_merge(first + cut[size_t(c)], first + cut[size_t(c + width)], first + cut[size_t(c + 2 * width)], cmp);
+    }
+}
+
 void sorted_unique(std::vector<int32_t> &v) {
-    std::sort(v.begin(), v.end());
+    parallel_sort(v.begin(), v.end(), [](int32_t a, int32_t b) { return a < b; });
     v.erase(std::unique(v.begin(), v.end()), v.end());
 }
 
@@ -43,6 +71,15 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
             err = fmt("cell_width[%lld] is not half of cell_width[%lld]", l, l - 1); return SG_ERR_ARG;
         }
     }
+    // SG_TIME_CREATE (debugging aid): print the duration of the phases of the layout build to stderr
+    const bool timing = std::getenv("SG_TIME_CREATE") != nullptr;
+    auto t_last = std::chrono::steady_clock::now();
+    auto lap = [&](const char *what) {
+        if (!timing) return;
+        const auto now = std::chrono::steady_clock::now();
+        std::fprintf(stderr, "  build_layout %-22s %8.1f ms\n", what, std::chrono::duration<double, std::milli>(now - t_last).count());
+        t_last = now;
+    };
     const int64_t N = n_patches * int64_t(P) * P;
     if (N >= (int64_t(1) << 29)) { err = "too many cells (limit 2^29)"; return SG_ERR_LAYOUT; }
 
@@ -76,21 +113,30 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
             if (leafset.count(patch_key(l, pi, pj))) return l;                // at `level` and coarser
         return -1;
     };
-    for (int64_t p = 0; p < n_patches && !cell_present; ++p) {
-        const sg_patch &q = patches[p];
-        const int64_t pi = q.i0 / P, pj = q.j0 / P;
-        if (q.level > 0 && covering_level(q.level - 1, pi >> 1, pj >> 1) >= 0) {
-            err = fmt("patch %lld (level %lld) lies inside a coarser leaf patch: leaves overlap", p, q.level);
+    if (!cell_present) {
+        int64_t bad = -1;
+        int unbalanced = 0;
+#pragma omp parallel for schedule(static) reduction(max : bad) reduction(| : unbalanced)
+        for (int64_t p = 0; p < n_patches; ++p) {                         // read-only look-ups in leafset
+            const sg_patch &q = patches[p];
+            const int64_t pi = q.i0 / P, pj = q.j0 / P;
+            if (q.level > 0 && covering_level(q.level - 1, pi >> 1, pj >> 1) >= 0) bad = std::max(bad, p);
+            if (q.level < 2) continue;                                    // a neighbour two levels coarser needs level >= 2
+            for (int dj = -1; dj <= 1; ++dj)
+                for (int di = -1; di <= 1; ++di) {
+                    if ((!di && !dj) || pi + di < 0 || pj + dj < 0) continue;
+                    const int c = covering_level(q.level, pi + di, pj + dj);
+                    if (c >= 0 && c < q.level - 1) unbalanced |= 1;
+                }
+        }
+        if (bad >= 0) {
+            err = fmt("patch %lld (level %lld) lies inside a coarser leaf patch: leaves overlap", bad, patches[bad].level);
             return SG_ERR_LAYOUT;
         }
-        for (int dj = -1; dj <= 1 && L.balanced; ++dj)
-            for (int di = -1; di <= 1; ++di) {
-                if ((!di && !dj) || pi + di < 0 || pj + dj < 0) continue;
-                const int c = covering_level(q.level, pi + di, pj + dj);
-                if (c >= 0 && c < q.level - 1) { L.balanced = false; break; }
-            }
+        L.balanced = unbalanced == 0;
     }
 
+    lap("validation");
     // ---- targets ------------------------------------------------------------------------------
     L.tkx.resize(N); L.tky.resize(N);
     {
@@ -123,11 +169,13 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     L.tX = L.tkx; sorted_unique(L.tX);
     L.tY = L.tky; sorted_unique(L.tY);
     L.itx.resize(N); L.ity.resize(N);
+#pragma omp parallel for schedule(static)
     for (int64_t c = 0; c < N; ++c) {
         L.itx[c] = int32_t(std::lower_bound(L.tX.begin(), L.tX.end(), L.tkx[c]) - L.tX.begin());
         L.ity[c] = int32_t(std::lower_bound(L.tY.begin(), L.tY.end(), L.tky[c]) - L.tY.begin());
     }
 
+    lap("targets");
     // ---- vertices: sort the 4N (corner key, cell, corner) records, merge equal keys ------------
     // corner id: 0 = NE (+), 1 = NW (-), 2 = SE (-), 3 = SW (+)
     struct Rec { uint64_t key; uint32_t cc; };
@@ -151,9 +199,11 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
         }
     }
     if (rec.empty()) { err = "no leaf cell present"; return SG_ERR_ARG; }
-    std::sort(rec.begin(), rec.end(), [](const Rec &a, const Rec &b) {
+    lap("corner records");
+    parallel_sort(rec.begin(), rec.end(), [](const Rec &a, const Rec &b) {
         return a.key != b.key ? a.key < b.key : a.cc < b.cc;
     });
+    lap("record sort");
     L.vkx.reserve(N + N / 8); L.vky.reserve(N + N / 8); L.adj.reserve(4 * (N + N / 8));
     for (size_t r = 0; r < rec.size();) {
         size_t e = r;
@@ -177,6 +227,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     L.Nv = int64_t(L.vkx.size());
     rec.clear(); rec.shrink_to_fit();
 
+    lap("vertex merge");
     // columns: vertices are already sorted by (kx, ky)
     for (int64_t v = 0; v < L.Nv; ++v) {
         if (v == 0 || L.vkx[v] != L.vkx[v - 1]) { L.colX.push_back(L.vkx[v]); L.colstart.push_back(int32_t(v)); }
@@ -186,7 +237,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     // rows: permutation sorted by (ky, kx)
     L.rowperm.resize(L.Nv);
     for (int64_t v = 0; v < L.Nv; ++v) L.rowperm[v] = int32_t(v);
-    std::sort(L.rowperm.begin(), L.rowperm.end(), [&](int32_t a, int32_t b) {
+    parallel_sort(L.rowperm.begin(), L.rowperm.end(), [&](int32_t a, int32_t b) {
         return L.vky[a] != L.vky[b] ? L.vky[a] < L.vky[b] : L.vkx[a] < L.vkx[b];
     });
     for (int64_t r = 0; r < L.Nv; ++r) {
@@ -195,6 +246,7 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     }
     L.rowstart.push_back(int32_t(L.Nv));
 
+    lap("columns and rows");
     // chunks: cut every column into runs of kChunk vertices; pad the last run of a column with -1
     for (size_t c = 0; c + 1 < L.colstart.size(); ++c)
         for (int32_t s = L.colstart[c]; s < L.colstart[c + 1]; s += kChunk) {
@@ -211,15 +263,23 @@ int build_layout(HostLayout &L, int n_levels, const double *cell_width, double x
     // cheap necessary check on the lattice -- both coordinates of a target being vertex coordinates is
     // only possible if some vertex lies inside a leaf, i.e. an overlap the patch test did not see.
     {
-        std::unordered_set<uint64_t> vset;
-        vset.reserve(size_t(L.Nv) * 2);
-        for (int64_t v = 0; v < L.Nv; ++v) vset.insert((uint64_t(L.vkx[v]) << 32) | uint32_t(L.vky[v]));
-        for (int64_t c = 0; c < N; ++c)
-            if ((!cell_present || cell_present[c]) && vset.count((uint64_t(L.tkx[c]) << 32) | uint32_t(L.tky[c]))) {
-                err = fmt("cell %lld: centre coincides with a vertex of another leaf: leaves overlap", c);
-                return SG_ERR_LAYOUT;
-            }
+        // the vertices are sorted by (kx, ky): look the target's position up in its column
+        int64_t bad = -1;
+#pragma omp parallel for schedule(static) reduction(max : bad)
+        for (int64_t c = 0; c < N; ++c) {
+            if (cell_present && !cell_present[c]) continue;
+            const auto cx = std::lower_bound(L.colX.begin(), L.colX.end(), L.tkx[c]);
+            if (cx == L.colX.end() || *cx != L.tkx[c]) continue;
+            const size_t col = size_t(cx - L.colX.begin());
+            const auto b0 = L.vky.begin() + L.colstart[col], b1 = L.vky.begin() + L.colstart[col + 1];
+            if (std::binary_search(b0, b1, L.tky[c])) bad = std::max(bad, c);
+        }
+        if (bad >= 0) {
+            err = fmt("cell %lld: centre coincides with a vertex of another leaf: leaves overlap", bad);
+            return SG_ERR_LAYOUT;
+        }
     }
+    lap("chunks and vertex check");
     return SG_OK;
 }
 
