@@ -246,7 +246,7 @@ def run_ours(args):
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2001_02765_b200 import SgDisk, measure_fp64_peak, shard_range
+    from paper_2001_02765_b200 import SgDisk, measure_fp64_peak, measure_fp64_mma_peak, shard_range
     from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
     from workloads import make_config, expected_counts
 
@@ -323,6 +323,7 @@ def run_ours(args):
         torch.cuda.current_stream().synchronize()      # the caller holds the result on the host
 
     peak_tflops, peak_winstr = measure_fp64_peak(local)
+    dmma_tflops, dmma_mixed_tflops = measure_fp64_mma_peak(local)
 
     # ---- device-resident timing -------------------------------------------------------------------
     def timed_resident(steps, warmup):
@@ -435,6 +436,10 @@ def run_ours(args):
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": args.steps * (sd_launches + f_launches),
             "clocks": clocks, "roofline": roofline,
+            "fp64_probes": {"dfma_tflops": peak_tflops, "mma_m8n8k4_f64_tflops": dmma_tflops,
+                            "mma_interleaved_with_dfma_total_tflops": dmma_mixed_tflops,
+                            "what": "micro-benchmarks outside the timed region (sg_measure_fp64_peak, "
+                                    "sg_measure_fp64_mma_peak): FP64 tensor-core MMA does not add to the DFMA rate"},
         }
         if direct_run is not None:
             d_total, d_kms, _, d_model = direct_run

@@ -51,3 +51,51 @@ def test_step_is_cuda_graph_capturable(mode):
         torch.cuda.synchronize()
         assert torch.equal(Fx, ref_a[0]) and torch.equal(Fy, ref_a[1])
         assert not torch.equal(ref_a[0], got_b[0])
+
+
+def test_lattice_slope_step_and_regrouped_step_are_capturable():
+    """The round-2 paths inside a CUDA graph: (a) slope terms in lattice mode on a three-level P = 16 nest (three
+    function-lattice planes, forked pair-class streams, finalise_lin), (b) a regrouped zone-wise quadtree (P = 1: scatter
+    into block order, inner context, gather).  Replay with new field contents equals the eager result bit for bit."""
+    import torch
+    from paper_2001_02765_b200 import SgDisk
+    from workloads import paper_ilr_layout
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required")
+    rng = np.random.default_rng(1)
+    for case in ("slopes", "regrouped"):
+        lay = nested_layout(3, 64, 4.0, 16) if case == "slopes" else paper_ilr_layout(64, 3)
+        x, y, _ = cell_centres(lay)
+        sigma = kuzmin_sigma(x, y, a=0.3)
+        g = -3.0 * sigma / (x * x + y * y + 0.09)
+        fields_a = [sigma, g * x, g * y]
+        fields_b = [f * (1.0 + 0.1 * rng.uniform(-1, 1, sigma.size)) for f in fields_a]
+        n_f = 3 if case == "slopes" else 1
+        with SgDisk.from_layout(lay, device=0) as d:
+            d.set_interaction_mode("lattice")
+            bufs = [torch.as_tensor(f).cuda() for f in fields_a[:n_f]]
+            Fx = torch.empty(lay.n_cells, dtype=torch.float64, device="cuda")
+            Fy = torch.empty_like(Fx)
+
+            def step():
+                if n_f == 3:
+                    d.set_density_linear(*bufs)
+                else:
+                    d.set_density(bufs[0])
+                d.force(Fx, Fy)
+            step()                                              # warm-up (first slope call allocates)
+            torch.cuda.synchronize()
+            ref_a = (Fx.clone(), Fy.clone())
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr):
+                step()
+            for b, f in zip(bufs, fields_b):
+                b.copy_(torch.as_tensor(f))
+            gr.replay()
+            torch.cuda.synchronize()
+            got_b = (Fx.clone(), Fy.clone())
+            step()
+            torch.cuda.synchronize()
+            assert torch.equal(got_b[0], Fx) and torch.equal(got_b[1], Fy), case
+            assert not torch.equal(got_b[0], ref_a[0]), case
+            assert bool(torch.isfinite(Fx).all()) and bool(torch.isfinite(Fy).all())

@@ -12,7 +12,7 @@ import torch.multiprocessing as mp
 
 import oracle
 from paper_2001_02765_b200 import SgDisk
-from paper_2001_02765_b200.sharding import all_gather_slices, shard_range
+from paper_2001_02765_b200.sharding import all_gather_slices, lattice_patch_costs, shard_range, shard_range_by_cost
 from workloads import cell_rects, make_config
 
 
@@ -57,3 +57,31 @@ def test_two_rank_target_sharding(tmp_path):
     idx = np.arange(n_targets)
     fx, fy, _ = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64", n_threads=2)
     assert np.array_equal(a[0], fx) and np.array_equal(a[1], fy)
+
+
+def _worker_cost(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from workloads import nested_layout
+        lay = nested_layout(4, 64, 8.0, 16)                  # four levels: coarse patches cost more (far pairs)
+        costs = lattice_patch_costs(lay.patches[:, 0])
+        ranges = [shard_range_by_cost(costs, lay.P * lay.P, r, world) for r in range(world)]
+        first, count = ranges[rank]
+        with SgDisk.from_layout(lay, device=-1) as d:        # host-only context: bookkeeping only
+            d.set_target_range(first, count)
+        local = torch.arange(first, first + count, dtype=torch.float64)      # every target's own index
+        full = all_gather_slices(local, lay.n_cells, ranges=ranges)
+        assert torch.equal(full, torch.arange(lay.n_cells, dtype=torch.float64))
+        np.save(os.path.join(out_dir, f"r{rank}.npy"), np.array([first, count]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_cost_based_slices(tmp_path):
+    """The lattice-mode partition (whole patches, balanced estimated cost, unequal counts) through the ragged gather."""
+    port = _free_port()
+    mp.spawn(_worker_cost, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    a, b = np.load(tmp_path / "r0.npy"), np.load(tmp_path / "r1.npy")
+    assert a[0] == 0 and a[0] + a[1] == b[0] and a[1] % 256 == 0 and a[1] != b[1]
