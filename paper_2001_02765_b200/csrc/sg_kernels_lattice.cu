@@ -82,6 +82,12 @@ constexpr int kLatAuxBytes = kChunkOffsets * 8 * 4      // sB: source patch of (
                              + 8 * 8 + 8 * 4            // full[] mbarriers, done[] counters
                              + 16 * 4 + 8 * 4;          // patch positions of the group, item / live count
 // dynamic shared memory per CTA with two CTAs per SM: (228 KB - 2 x 1 KB reserved) / 2, minus a little static room
+// Deepest ring.  4 stages of the same-level class leave ~45 KB of the SM's 256 KB to L1, where the warps' weight rows
+// live (16 warps x 2.4 KB); with 6 stages the L1 hit rate of the weight loads was 63 % and cfg 5 ran 1.3 % slower, and
+// the AMR configs gained nothing from the deeper ring (cfg 4: 40.1 vs 40.3 ms).
+#ifndef SG_LAT_KMAX
+#define SG_LAT_KMAX 4
+#endif
 constexpr int kLatSmemBudget = 115712 - 256;
 
 // A stage of the ring holds a whole table (classes at most one level apart) or a SUB-BLOCK of its rows: the 80-row
@@ -99,7 +105,7 @@ struct LatCls {
     static constexpr int SLOT_ENTRIES = SLOT_ROWS * C::TROW;
     static constexpr int STAGE_BYTES = SLOT_ENTRIES * 16;
     static constexpr int K_FIT = (kLatSmemBudget - kLatAuxBytes) / STAGE_BYTES;
-    static constexpr int K = K_FIT < 1 ? 1 : (K_FIT > 6 ? 6 : K_FIT);        // ring depth: 6, 3, 3, 3, 4
+    static constexpr int K = K_FIT < 1 ? 1 : (K_FIT > SG_LAT_KMAX ? SG_LAT_KMAX : K_FIT);        // ring depth: 4, 3, 3, 3, 4
     static constexpr size_t smem = size_t(K) * STAGE_BYTES + kLatAuxBytes;
 };
 
