@@ -89,6 +89,10 @@ def parse_args():
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config list (all five configs)")
     ap.add_argument("--mode", default="auto", choices=["auto", "direct", "lattice"],
                     help="S3 algorithm: direct pair sum, lattice-offset reuse, or auto (lattice when the layout allows)")
+    ap.add_argument("--paper-layout", default=None, metavar="RULE:DISK:L:NK",
+                    help="instead of a BASELINE.json config: one of the paper's own zone-wise quadtrees, e.g. ILR:D2:3:1024 "
+                         "(PAPER.md:164, Tables 3-9; 1 x 1 patches, regrouped into 16 x 16 blocks in lattice mode) with the "
+                         "paper's D2 / D22 disk; add --slopes for the full second-order method the paper times")
     ap.add_argument("--slopes", action="store_true",
                     help="time the first-order path (sg_set_density_linear); default is the zeroth-order hot path")
     return ap.parse_args()
@@ -176,15 +180,33 @@ def per_config_measurement(torch, device, flush, cfg, nominal_tflops, steps=5, w
                          "executed_over_algorithmic": mdl["executed_evaluations"] / max(1.0, mdl["pair_evaluations"])}}
 
 
-def workload_name(cfg: int) -> str:
+def workload_name(cfg) -> str:
     from workloads import CONFIG_NAMES
-    return CONFIG_NAMES[cfg]
+    return CONFIG_NAMES[cfg] if isinstance(cfg, int) else str(cfg)
+
+
+def load_workload(args):
+    """(workload key, layout, sigma, slopes or None): a BASELINE.json config, or one of the paper's quadtrees."""
+    from workloads import make_config, expected_counts
+    if args.paper_layout:
+        from workloads import paper_ilr_layout, paper_vlr_layout, d2_sigma, d2_slopes, d22_sigma, d22_slopes
+        from workloads.configs import cell_centres
+        rule, disk, L, Nk = args.paper_layout.split(":")
+        lay = (paper_ilr_layout if rule.upper() == "ILR" else paper_vlr_layout)(int(Nk), int(L), disk)
+        x, y, _ = cell_centres(lay)
+        if disk == "D2":
+            return f"paper_{rule}_{disk}_L{L}_Nk{Nk}", lay, d2_sigma(x, y, 0.5), d2_slopes(x, y, 0.5)
+        return f"paper_{rule}_{disk}_L{L}_Nk{Nk}", lay, d22_sigma(x, y), d22_slopes(x, y)
+    lay, sigma = make_config(args.config)
+    exp = expected_counts(args.config)
+    assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"], "frozen layout changed"
+    return args.config, lay, sigma, None
 
 
 # --------------------------------------------------------------------------------------------------
 # CPU legs: the oracle as it stands (oracle/sg_oracle.c, double build, OpenMP over targets)
 # --------------------------------------------------------------------------------------------------
-def oracle_sample_rate(lay, sigma, seconds: float, seed: int = 99):
+def oracle_sample_rate(lay, sigma, seconds: float, seed: int = 99, slopes=None):
     """Time the oracle on a bounded, seeded sample of targets of this workload (every sampled target is
     summed over ALL N leaves, so pairs/s does not depend on the sample size).  Returns
     (pairs_per_s, threads, n_targets, elapsed_s)."""
@@ -196,14 +218,15 @@ def oracle_sample_rate(lay, sigma, seconds: float, seed: int = 99):
     n_cal = min(lay.n_cells, max(2 * cores, 8))
     idx = sample_targets(lay, n_cal, seed)
     t0 = time.perf_counter()
-    _, _, threads = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64")
+    kw = {} if slopes is None else {"dx": slopes[0], "dy": slopes[1]}
+    _, _, threads = oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64", **kw)
     dt = max(time.perf_counter() - t0, 1e-6)
     rate = idx.size * lay.n_cells / dt
     n = int(min(lay.n_cells, max(n_cal, seconds * rate / lay.n_cells)))
     n = max(threads, (n // threads) * threads)
     idx = sample_targets(lay, min(n, lay.n_cells), seed + 1)
     t0 = time.perf_counter()
-    oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64")
+    oracle.force(r, sigma, r["kxc"][idx], r["kyc"][idx], lay.unit, precision="f64", **kw)
     dt = time.perf_counter() - t0
     return idx.size * lay.n_cells / dt, threads, int(idx.size), dt
 
@@ -213,8 +236,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from workloads import make_config
-    lay, sigma = make_config(args.config)
+    wkey, lay, sigma, _ = load_workload(args)
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     rates, threads, n_t = [], 1, 0
     for i in range(args.warmup + args.steps):
@@ -230,7 +252,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps),
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.config), "n_cells": lay.n_cells,
+        "config": {"workload": workload_name(wkey), "n_cells": lay.n_cells,
                    "pairs_per_evaluation": lay.n_cells ** 2},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -265,14 +287,12 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    lay, sigma = make_config(args.config)
-    exp = expected_counts(args.config)
-    assert lay.n_cells == exp["n_cells"] and lay.n_patches == exp["n_patches"], "frozen layout changed"
+    wkey, lay, sigma, paper_slopes = load_workload(args)
     N = lay.n_cells
-    lattice = args.mode != "direct" and (lay.P == 16 or (lay.P == 8 and not args.slopes))
+    lattice = args.mode != "direct" and (lay.P in (1, 2, 4, 16) or (lay.P == 8 and not args.slopes))
     if args.mode == "lattice" and not lattice:
-        raise SystemExit("--mode lattice needs 16x16 patches (8x8 for the zeroth-order path only)")
-    if lattice:
+        raise SystemExit("--mode lattice needs patches of 1, 2, 4 or 16 cells (8x8 for the zeroth-order path only)")
+    if lattice and lay.P == 16:
         # lattice mode works on whole patches and a target's cost depends on its level: split by estimated cost
         first, count = shard_range_by_cost(lattice_patch_costs(lay.patches[:, 0]), lay.P * lay.P, rank, world)
     else:
@@ -285,7 +305,9 @@ def run_ours(args):
     info = d.layout_info()
 
     fields = [sigma]
-    if args.slopes:
+    if args.slopes and paper_slopes is not None:
+        fields += list(paper_slopes)                # exact Taylor coefficients of the paper's disks (R10)
+    elif args.slopes:
         # first-order Taylor coefficients of the smooth Kuzmin profile every bench config is
         # built on (cfg 3/4: centred differences of the cell samples along the library's own rows would need the
         # neighbour links; analytic slopes of the base profile are the paper's choice, R10)
@@ -349,11 +371,13 @@ def run_ours(args):
         return total, kms, clk, mdl
 
     d.set_interaction_mode("lattice" if lattice else "direct")
+    set_density()                                   # (a regrouped layout wants its density after the mode is chosen)
     sd_launches, f_launches = d.launch_counts()
     ms_total, k_ms, clocks, model = timed_resident(args.steps, max(3, args.warmup))
     direct_run = None
-    if lattice and world == 1:
+    if lattice and world == 1 and N <= 2200000:
         # the north_star kernel (every pair: sqrt + 2 ln) on the same workload, same run, for its roofline line
+        # (skipped above 2.2 M cells, where six direct steps would take minutes)
         d.set_interaction_mode("direct")
         direct_run = timed_resident(DIRECT_LEG_STEPS, 3)
         d.set_interaction_mode("lattice")
@@ -408,14 +432,14 @@ def run_ours(args):
             direct_name = "interaction_lin_kernel<4>"
         else:
             direct_name = "interaction_kernel<4>" if count > 16384 else "interaction_kernel<1>"
-        direct_traffic = measured_traffic(workload_name(args.config), direct_name) if world == 1 else None
+        direct_traffic = measured_traffic(workload_name(wkey), direct_name) if world == 1 else None
         if lattice:
             lattice_name = ("lattice_corr_kernel<0> (same-level pairs; <1>..<4> for pairs one and two levels apart"
                             + ("; three planes per offset: slope terms)" if args.slopes else ")"))
             if lay.P == 8:
                 lattice_name = "patch_interaction_kernel<8>"
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, lattice_name,
-                                   measured_traffic(workload_name(args.config) + ("+slopes" if args.slopes else ""),
+                                   measured_traffic(workload_name(wkey) + ("+slopes" if args.slopes else ""),
                                                     lattice_name) if world == 1 else None)
         else:
             roofline = roofline_of(model, k_ms_avg, ms_total / args.steps, direct_name, direct_traffic)
@@ -423,7 +447,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config), "n_cells": N, "n_vertices": info["n_vertices"],
+            "config": {"workload": workload_name(wkey), "n_cells": N, "n_vertices": info["n_vertices"],
                        "pairs_per_evaluation": pairs,
                        "order": "sigma0 + slope terms (Eq. 6)" if args.slopes else "sigma0 (north_star hot path)",
                        "interaction_mode": ("lattice-offset reuse (SG_MODE_LATTICE): precomputed function lattices "
@@ -451,7 +475,7 @@ def run_ours(args):
                 "value": pairs * DIRECT_LEG_STEPS / (d_total * 1e-3), "unit": UNIT, "ms_per_step": d_total / DIRECT_LEG_STEPS,
                 "steps": DIRECT_LEG_STEPS, "warmup": 3,
                 "roofline": roofline_of(d_model, d_k, d_total / DIRECT_LEG_STEPS, direct_name, direct_traffic)}
-        if world == 1 and not args.slopes and not args.no_per_config:
+        if world == 1 and not args.slopes and not args.no_per_config and not args.paper_layout:
             # north_star: "report throughput on synthetic disks shaped like the paper's workloads": all five configs,
             # same calls, same run (the headline workload's own entry repeats the numbers above)
             line["per_config"] = []
@@ -469,7 +493,8 @@ def run_ours(args):
                 else:
                     line["per_config"].append(per_config_measurement(torch, local, flush, cfg, nominal_tflops))
         if not args.no_cpu_baseline and world == 1:
-            rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds)
+            rate, threads, n_t, dt = oracle_sample_rate(lay, sigma, args.cpu_baseline_seconds,
+                                                        slopes=fields[1:] if args.slopes else None)
             line["cpu_baseline"] = {
                 "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
                 "sample": f"{n_t} seeded targets (stratified by level), each summed over all {N} leaves; "
