@@ -129,17 +129,27 @@ int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
 int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 
 /*
- * How sg_force evaluates the O(N^2) interaction sum (S3) of the zeroth-order path.
+ * How sg_force evaluates the O(N^2) interaction sum (S3).  Same sum and same tolerances in every mode (
+ * the paper rules out FFT on AMR, :267, :295 -- lattice mode is the patch-wise counterpart that needs no uniform grid).
  *   SG_MODE_DIRECT   every (target, vertex) pair: 1 sqrt + 2 ln (the north_star kernel; always available; default)
- *   SG_MODE_LATTICE  lattice-offset reuse: per (target patch, source patch) the pair function
- *                    is tabulated once on the patch pair's offset lattice and the pairs reduce to 2 FMA each;
- *                    Needs P = 8 or 16
- *                    (SG_ERR_ARG otherwise).  Same sum, same tolerances; the slope path always runs DIRECT.
- *                    P = 16 runs the register-blocked kernels that share one offset table per CTA (patch pairs
- *                    up to two levels apart; farther pairs are summed directly); P = 8 a lighter
- *                    one-target-per-thread kernel (pairs up to one level apart by table).
- *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but SG_ERR_ARG unless the register-blocked kernels are
- *                    available (P = 16).  For tests and profiling.
+ *   SG_MODE_LATTICE  lattice-offset reuse: for a (target patch, source patch) pair the pair function
+ *                    depends on the lattice offset only, so the pairs reduce to 2 FMA each against a table.
+ *                    P = 16: the tables are windows of per-layout function lattices that this call builds ONCE (device
+ *                      memory; budget a quarter of the device, SG_LATTICE_TABLE_MIB overrides) and that sg_force
+ *                      streams by TMA -- no square root or logarithm is evaluated in sg_force for patch pairs up to two
+ *                      levels apart (farther pairs are summed directly).  Covers the slope path of
+ *                      sg_set_density_linear too (three table planes, 6 FMA per pair).  Over the budget: as
+ *                      SG_MODE_LATTICE_INCTA, and the slope path runs direct.
+ *                    P = 1, 2, 4 (e.g. the paper's zone-wise quadtrees): the leaves are regrouped into padded 16 x 16
+ *                      blocks of an inner context (needs a device); set the density AFTER selecting the mode, an
+ *                      sg_force with a density set before returns SG_ERR_STATE.
+ *                    P = 8: a lighter one-target-per-thread kernel with tables built on the fly (pairs up to one level
+ *                      apart by table; zeroth-order path only, the slope path runs direct).
+ *                    Other P: SG_ERR_ARG.
+ *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but SG_ERR_ARG unless P = 16.  For tests and profiling.
+ *   SG_MODE_LATTICE_INCTA    P = 16, offset tables built inside the CTAs at every sg_force (the round-1 kernels; no
+ *                    table memory; zeroth-order path only).  Bit-identical to SG_MODE_LATTICE.
+ * Host-synchronous: may allocate and build tables; not to be called during stream capture.
  */
 #define SG_MODE_DIRECT  0
 #define SG_MODE_LATTICE 1
