@@ -890,6 +890,14 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
             note(cudaStreamWaitEvent(st, c->fork_ev, 0), "cudaStreamWaitEvent(fork)");
             return st;
         };
+        if (sp.blocked && sp.far) {
+            // pairs >= 3 levels apart, directly: the longest launch of a deep hierarchy goes first, so that the short
+            // table classes fill in beside and after it (its partial sums are the LAST slots of `part`)
+            double *far_part = part + int64_t(offset_classes(po)) * po.n_split * 2 * c->count;
+            launch_patch_far(c->linear, c->dev, c->patch, c->linear ? c->lat.wS : c->patch.wQ, sp.pp, c->first, c->count, far_part,
+                             on_stream(n_launch));
+            ++n_launch;
+        }
         if (sp.blocked)
             for (int v = 0; v < kOffClasses; ++v)
                 if (po.variant[v]) {
@@ -905,11 +913,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
                         if (e != cudaSuccess) { first_err = e; where = std::string(sp.fn ? "lattice_corr_kernel<" : "patch_offset_kernel<") + std::to_string(v) + ">"; }
                     }
                 }
-        if (sp.blocked && sp.far) {                            // pairs >= 3 levels apart, directly
-            launch_patch_far(c->linear, c->dev, c->patch, c->linear ? c->lat.wS : c->patch.wQ, sp.pp, c->first, c->count, part,
-                             on_stream(n_launch));
-            ++n_launch;
-        } else if (!sp.blocked) {                              // P = 8: everything in the generic kernel
+        if (!sp.blocked) {                              // P = 8: everything in the generic kernel
             launch_patch_interaction(c->dev, c->patch, sp.pp, c->first, c->count, part, 0, on_stream(n_launch));
             ++n_launch;
         }
