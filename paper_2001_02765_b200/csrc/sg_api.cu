@@ -33,6 +33,7 @@ struct sg_ctx {
     std::vector<PatchGroup> patch_groups;   // the three group lists back to back (offset_group_list)
     int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
     bool use_patch = false;      // sg_set_interaction_mode
+    bool neutral_weights = false; // SG_LATTICE_NEUTRAL_WEIGHTS at sg_create: own-cell per-patch weights (sg_kernels_patch.cu)
     bool force_incta = false;    // SG_MODE_LATTICE_INCTA: offset tables built inside the CTAs even if the lattices exist
     LatticeArrays lat;           // precomputed function lattices of the pair classes (sg_kernels_lattice.cu)
     std::vector<FnLattice> lat_meta;        // host copy, [n_levels * kOffClasses]
@@ -530,6 +531,12 @@ int upload_patches(sg_ctx *c) {
                 if (v >= 0 && e / P1 == h.P) pflags[size_t(p)] |= 1;
                 if (v >= 0 && e / P1 < h.P && e % P1 == h.P) pflags[size_t(p)] |= 2;
             }
+        // SG_LATTICE_NEUTRAL_WEIGHTS (read at sg_create): per-patch weights from the patch's own cells on all 17 x 17
+        // vertices instead of owned deduplicated weights on 16 x 16 -- 7 % slower on cfg 5, but every patch is neutral
+        // and the rounding error on steep, deep hierarchies drops (12 M-leaf config 4: 1.4e-12 -> 5e-14 of max|F|;
+        // DESIGN.md 6c).  Zeroth-order path; the slope path keeps the owned weights (all rows and columns correlated).
+        c->neutral_weights = std::getenv("SG_LATTICE_NEUTRAL_WEIGHTS") != nullptr;
+        if (c->neutral_weights) for (auto &f : pflags) f = 3;
         c->patch_flags = pflags;
         if ((rc = upload(c, &pa.pflags, pflags))) return rc;
         if ((rc = upload(c, &pa.pvmap, pv))) return rc;
@@ -770,7 +777,10 @@ int sg_set_density(sg_ctx *c, const double *sigma_dev, void *cuda_stream) {
     SG_CUDA(c, guard.err);
     launch_vertex_weights(c->dev, sigma_dev, s);
     launch_line_tables(c->dev, s);
-    if (c->patch.enabled) launch_patch_weights(c->patch, c->dev.w, s);
+    if (c->patch.enabled) {
+        if (c->neutral_weights) launch_patch_weights_owncell(c->patch, sigma_dev, s);
+        else launch_patch_weights(c->patch, c->dev.w, s);
+    }
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = false;

@@ -60,6 +60,34 @@ __global__ void patch_weights_kernel(const double *__restrict__ w, const int32_t
     }
 }
 
+// Alternative per-patch weights (SG_LATTICE_NEUTRAL_WEIGHTS, sg_api.cu): the corner sums of the patch's OWN cells only, on
+// all (P+1)^2 vertices.  Every patch is then neutral (its weights sum to zero, and so do their first moments), so a
+// patch pair contributes a small quadrupole-like number instead of a monopole that only cancels against the
+// neighbouring patches' sums: less rounding on steep, deep hierarchies, at the price of 289 instead of 256 vertices.
+__global__ void patch_weights_owncell_kernel(const double *__restrict__ sigma, double *__restrict__ wP, double *__restrict__ wQ,
+                                             int P, int wstride) {
+    const int p = blockIdx.x;
+    const double *s = sigma + int64_t(p) * P * P;
+    for (int e = threadIdx.x; e < wstride; e += blockDim.x) {
+        double w = 0.0;
+        if (e < (P + 1) * (P + 1)) {
+            const int i = e % (P + 1), j = e / (P + 1);
+            if (i >= 1 && j >= 1) w += s[(j - 1) * P + (i - 1)];
+            if (i < P && j >= 1) w -= s[(j - 1) * P + i];
+            if (i >= 1 && j < P) w -= s[j * P + (i - 1)];
+            if (i < P && j < P) w += s[j * P + i];
+            if (wQ) {
+                wQ[int64_t(p) * kPatchQStride + j * (P + 2) + i] = w;
+                if (i == P) wQ[int64_t(p) * kPatchQStride + j * (P + 2) + P + 1] = 0.0;
+            }
+        }
+        wP[int64_t(p) * wstride + e] = w;
+    }
+}
+void launch_patch_weights_owncell(const PatchArrays &pa, const double *sigma, cudaStream_t s) {
+    patch_weights_owncell_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, pa.wP, pa.wQ, pa.P, pa.wstride);
+}
+
 void launch_patch_weights(const PatchArrays &pa, const double *w, cudaStream_t s) {
     patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(w, pa.pvmap, pa.wP, pa.wQ, pa.P, pa.wstride, 1, 0);
 }

@@ -368,3 +368,23 @@ def test_regrouped_paper_quadtree_at_scale(torch_cuda):
     assert t_dir >= 5.0 * t_lat, (t_dir, t_lat)                    # >= 5x the direct time
     idx = sample_targets(lay, 96, 3071)
     check(gx[idx], gy[idx], *oracle_force(lay, sigma, idx))
+
+
+def test_neutral_patch_weights_variant(torch_cuda, monkeypatch):
+    """SG_LATTICE_NEUTRAL_WEIGHTS: per-patch weights from the patch's own cells on all 17 x 17 vertices (every patch
+    neutral) instead of owned deduplicated weights on 16 x 16.  Same sum: both variants within the gates on a steep
+    profile (config 4's tanh-tapered disk) over an irregular four-level hierarchy, all targets, and on P = 8."""
+    from workloads.configs import _ppd_sigma
+    lay = random_refined_layout(21, 5, 16, 4, 0.4, half_extent=1.2)
+    x, y, _ = cell_centres(lay)
+    sigma = _ppd_sigma(x, y)
+    ref = oracle_force(lay, sigma, np.arange(lay.n_cells))
+    a = gpu_force(torch_cuda, lay, sigma, "lattice")
+    check(a[0], a[1], *ref)
+    monkeypatch.setenv("SG_LATTICE_NEUTRAL_WEIGHTS", "1")
+    b = gpu_force(torch_cuda, lay, sigma, "lattice")
+    check(b[0], b[1], *ref)
+    assert not (np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]))       # the variant really ran
+    lay8, sig8 = make_config(2)
+    g = gpu_force(torch_cuda, lay8, sig8, "lattice")
+    check(g[0], g[1], *oracle_force(lay8, sig8, np.arange(lay8.n_cells)))
