@@ -297,9 +297,9 @@ int ensure_fn_lattices(sg_ctx *c, int n_planes) {
 
 // Source vertices the lattice kernels run through per target: (P + 1)^2 per patch in the generic kernel; in the
 // offset-table kernels (P = 16) vertex row 16 / column 16 of a patch only where it owns vertices there (pflags).
-double executed_patch_vertices(const sg_ctx *c) {
+double executed_patch_vertices(const sg_ctx *c, bool all_vertices = false) {
     const int P = c->host.P;
-    if (c->patch_flags.size() != c->host.patches.size()) return double(c->host.patches.size()) * double((P + 1) * (P + 1));
+    if (all_vertices || c->patch_flags.size() != c->host.patches.size()) return double(c->host.patches.size()) * double((P + 1) * (P + 1));
     double n = 0.0;
     for (int32_t f : c->patch_flags) n += double(P + (f & 1)) * double(P + ((f >> 1) & 1));
     return n;
@@ -823,7 +823,16 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
         if ((rc = reserve_partials(c))) return rc;
     }
     launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
-    if (c->lat.wS) launch_patch_weights_lin(c->patch, l.wl, c->lat.wS, s);
+    if (c->lat.wS) {
+        // Slope path in lattice mode: own-cell (neutral) per-patch weights on all 17 x 17 vertices when the lattice is
+        // large, owned deduplicated weights on 16 x 16 (7 % faster) otherwise.  The rounding error of the owned weights
+        // grows with the square of the lattice extent in the slope path (8e-13 at an extent of 4,096 lattice
+        // units, 3.5e-12 at 8,192, 1.4e-11 at 16,384 on the paper's AMR(3, D22) quadtrees; neutral weights: 1.5e-13,
+        // 3.9e-13, ~1e-12), so the switch is at 4,096.  SG_LATTICE_NEUTRAL_WEIGHTS forces the neutral weights.
+        c->lat.lin_neutral = c->neutral_weights || c->host.extent > 4096;
+        if (c->lat.lin_neutral) launch_patch_weights_lin_owncell(c->patch, sigma_dev, dx_dev, dy_dev, l.patch_hh, l.unit, c->lat.wS, s);
+        else launch_patch_weights_lin(c->patch, l.wl, c->lat.wS, s);
+    }
     SG_CUDA(c, cudaGetLastError());
     c->density_set = true;
     c->linear = true;
@@ -1178,7 +1187,7 @@ int sg_kernel_model(const sg_ctx *c, double *fp64_instr_per_pair, double *flops_
         // slope path in lattice mode: three planes, 6 DFMA per pair (sg_kernels_lattice.cu)
         if (fp64_instr_per_pair) *fp64_instr_per_pair = 6.0;
         if (flops_per_pair) *flops_per_pair = 12.0;
-        if (executed_evaluations) *executed_evaluations = double(c->count) * executed_patch_vertices(c);
+        if (executed_evaluations) *executed_evaluations = double(c->count) * executed_patch_vertices(c, c->lat.lin_neutral);
         return SG_OK;
     }
     if (sp.by_patch) {

@@ -115,7 +115,7 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                     const PatchGroup *__restrict__ groups, const int32_t *__restrict__ pmap,
                     const double *__restrict__ wq, int64_t w_plane_stride, const int32_t *__restrict__ pflags,
                     const double2 *__restrict__ fn,
-                    const FnLattice *__restrict__ meta, int n_planes, int n_groups, int n_split, int first_patch,
+                    const FnLattice *__restrict__ meta, int n_planes, int flags_or, int n_groups, int n_split, int first_patch,
                     int last_patch, int64_t first, int64_t count, double *__restrict__ part,
                     unsigned int *__restrict__ queue) {
     using C = OffCls<V>;
@@ -191,7 +191,7 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
         // the table T: correlate_patch, shared with patch_offset_kernel
         auto consume = [&](int b, int pl, int sub, const double2 *T) {
             const double2 *src = reinterpret_cast<const double2 *>(wq + int64_t(pl) * w_plane_stride + int64_t(b) * kPatchQStride);
-            const int flags = __ldg(pflags + b);
+            const int flags = __ldg(pflags + b) | flags_or;    // flags_or = 3: all 17 x 17 vertices (own-cell weights)
             if (V == kOffCoarserSrc4)            // slot row 0 = table row 16 sub; source rows 4 sub .. 4 sub + 3
                 correlate_patch<V>(T - 16 * sub * TROW, src, flags, l, h, ax, ay, 4 * sub, min(4 * sub + 3, P), 1);
             else if (V == kOffFinerSrc4)         // slot row 0 = stored row sub RPC; source rows sub, sub + 4, ...
@@ -304,7 +304,7 @@ void launch_lattice_corr_one(const DevLayout &d, const PatchArrays &pa, const La
     const double *wq = n_planes == 1 ? pa.wQ : la.wS;
     lattice_corr_kernel<V><<<grid, kOffWarps * 32, LatCls<V>::smem, s>>>(
         pa.info, pa.levels, groups, pa.pmap, wq, int64_t(pa.n_patches) * kPatchQStride, pa.pflags, la.fn, la.meta, n_planes,
-        n_groups, po.n_split, po.first_patch, po.last_patch, first, count, part, d.queue + 1 + V);
+        (n_planes > 1 && la.lin_neutral) ? 3 : 0, n_groups, po.n_split, po.first_patch, po.last_patch, first, count, part, d.queue + 1 + V);
 }
 
 void launch_lattice_corr(int V, const DevLayout &d, const PatchArrays &pa, const LatticeArrays &la, const OffsetPlan &po,

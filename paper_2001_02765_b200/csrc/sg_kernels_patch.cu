@@ -92,6 +92,47 @@ void launch_patch_weights(const PatchArrays &pa, const double *w, cudaStream_t s
     patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(w, pa.pvmap, pa.wP, pa.wQ, pa.P, pa.wstride, 1, 0);
 }
 
+// The slope-path counterpart of patch_weights_owncell_kernel: -W0, a, c of a patch vertex from the <= 4 cells of the
+// SAME patch, W0 = sum s (sigma + dx (xbar - x_c) + dy (ybar - y_c)), a = sum s dx, c = sum s dy (slopes per lattice
+// unit; xbar - x_c = +-hh), in the [17][18] layout.
+__global__ void patch_weights_lin_owncell_kernel(const double *__restrict__ sigma, const double *__restrict__ dx,
+                                                 const double *__restrict__ dy, const double *__restrict__ patch_hh,
+                                                 double unit, double *__restrict__ wS, int64_t plane_stride) {
+    constexpr int P = 16;
+    const int p = blockIdx.x;
+    const int64_t c0 = int64_t(p) * P * P;
+    const double hh = patch_hh[p];
+    for (int e = threadIdx.x; e < kPatchQStride; e += blockDim.x) {
+        const int i = e % (P + 2), j = e / (P + 2);
+        double W0 = 0.0, a = 0.0, c = 0.0;
+        if (i <= P) {
+            // cell (ci, cj) has the vertex as its NE (+), NW (-), SE (-), SW (+) corner
+            const int ci[4] = {i - 1, i, i - 1, i}, cj[4] = {j - 1, j - 1, j, j};
+            const double sg[4] = {1.0, -1.0, -1.0, 1.0};
+            const double ex[4] = {1.0, -1.0, 1.0, -1.0}, ey[4] = {1.0, 1.0, -1.0, -1.0};
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (ci[k] >= 0 && ci[k] < P && cj[k] >= 0 && cj[k] < P) {
+                    const int64_t cell = c0 + cj[k] * P + ci[k];
+                    const double dxl = dx[cell] * unit, dyl = dy[cell] * unit;
+                    W0 += sg[k] * (sigma[cell] + ex[k] * dxl * hh + ey[k] * dyl * hh);
+                    a += sg[k] * dxl;
+                    c += sg[k] * dyl;
+                }
+        }
+        const int64_t o = int64_t(p) * kPatchQStride + e;
+        wS[o] = -W0;
+        wS[plane_stride + o] = a;
+        wS[2 * plane_stride + o] = c;
+    }
+}
+
+void launch_patch_weights_lin_owncell(const PatchArrays &pa, const double *sigma, const double *dx, const double *dy,
+                                      const double *patch_hh, double unit, double *wS, cudaStream_t s) {
+    patch_weights_lin_owncell_kernel<<<pa.n_patches, 128, 0, s>>>(sigma, dx, dy, patch_hh, unit, wS,
+                                                                  int64_t(pa.n_patches) * kPatchQStride);
+}
+
 void launch_patch_weights_lin(const PatchArrays &pa, const double *wl, double *wS, cudaStream_t s) {
     patch_weights_kernel<<<pa.n_patches, 128, 0, s>>>(wl, pa.pvmap, nullptr, wS, pa.P, pa.wstride, 3,
                                                       int64_t(pa.n_patches) * kPatchQStride);

@@ -68,6 +68,8 @@ cudaError_t configure_patch_kernels(int P, int tab_entries);
 // w: flat deduplicated vertex weights (DevLayout::w); wl: {W0, a, c} per vertex of the slope path (LinArrays::wl)
 void launch_patch_weights(const PatchArrays &pa, const double *w, cudaStream_t s);
 void launch_patch_weights_owncell(const PatchArrays &pa, const double *sigma, cudaStream_t s);
+void launch_patch_weights_lin_owncell(const PatchArrays &pa, const double *sigma, const double *dx, const double *dy,
+                                      const double *patch_hh, double unit, double *wS, cudaStream_t s);
 void launch_patch_weights_lin(const PatchArrays &pa, const double *wl, double *wS, cudaStream_t s);
 // skip_near: patch pairs fewer than skip_near levels apart are skipped (done by patch_offset_kernel); 0 = none
 void launch_patch_interaction(const DevLayout &d, const PatchArrays &pa, const PatchPlan &pp, int64_t first,
