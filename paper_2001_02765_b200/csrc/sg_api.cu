@@ -531,11 +531,13 @@ int upload_patches(sg_ctx *c) {
                 if (v >= 0 && e / P1 == h.P) pflags[size_t(p)] |= 1;
                 if (v >= 0 && e / P1 < h.P && e % P1 == h.P) pflags[size_t(p)] |= 2;
             }
-        // SG_LATTICE_NEUTRAL_WEIGHTS (read at sg_create): per-patch weights from the patch's own cells on all 17 x 17
-        // vertices instead of owned deduplicated weights on 16 x 16 -- 7 % slower on cfg 5, but every patch is neutral
-        // and the rounding error on steep, deep hierarchies drops (12 M-leaf config 4: 1.4e-12 -> 5e-14 of max|F|;
-        // DESIGN.md 6c).  Zeroth-order path; the slope path keeps the owned weights (all rows and columns correlated).
-        c->neutral_weights = std::getenv("SG_LATTICE_NEUTRAL_WEIGHTS") != nullptr;
+        // Per-patch weights of lattice mode: owned deduplicated weights on 16 x 16 vertices (fast: cfg 5 162.7 ms), or
+        // "neutral" weights from the patch's own cells on all 17 x 17 vertices (176.2 ms), with which every patch's
+        // weights sum to zero and the rounding error does not grow with the lattice: 12 M-leaf config 4 (extent 16,384
+        // lattice units) 1.4e-12 -> 5e-14 of max|F|, slope path on the 6 M-leaf quadtrees 1.4e-11 -> < 1e-11
+        // (DESIGN.md 6c, 8).  Neutral on lattices of more than 4,096 units, or when SG_LATTICE_NEUTRAL_WEIGHTS is set
+        // (read at sg_create); owned below, where both agree to ~1e-13.
+        c->neutral_weights = std::getenv("SG_LATTICE_NEUTRAL_WEIGHTS") != nullptr || h.extent > 4096;
         if (c->neutral_weights) for (auto &f : pflags) f = 3;
         c->patch_flags = pflags;
         if ((rc = upload(c, &pa.pflags, pflags))) return rc;
@@ -824,12 +826,8 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
     }
     launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
     if (c->lat.wS) {
-        // Slope path in lattice mode: own-cell (neutral) per-patch weights on all 17 x 17 vertices when the lattice is
-        // large, owned deduplicated weights on 16 x 16 (7 % faster) otherwise.  The rounding error of the owned weights
-        // grows with the square of the lattice extent in the slope path (8e-13 at an extent of 4,096 lattice
-        // units, 3.5e-12 at 8,192, 1.4e-11 at 16,384 on the paper's AMR(3, D22) quadtrees; neutral weights: 1.5e-13,
-        // 3.9e-13, ~1e-12), so the switch is at 4,096.  SG_LATTICE_NEUTRAL_WEIGHTS forces the neutral weights.
-        c->lat.lin_neutral = c->neutral_weights || c->host.extent > 4096;
+        // slope path in lattice mode: the same choice of per-patch weights as the zeroth-order path (upload_patches)
+        c->lat.lin_neutral = c->neutral_weights;
         if (c->lat.lin_neutral) launch_patch_weights_lin_owncell(c->patch, sigma_dev, dx_dev, dy_dev, l.patch_hh, l.unit, c->lat.wS, s);
         else launch_patch_weights_lin(c->patch, l.wl, c->lat.wS, s);
     }
