@@ -334,3 +334,31 @@ def test_paper_tables4_6_D22_Linf_on_gpu(torch_cuda, golden, rule, L, Nk):
                 assert abs(got - float(printed)) <= 0.01 * float(printed), (got, row)
             else:
                 assert _agree_3_digits(got, printed), (got, row)
+
+
+@pytest.mark.parametrize("Nk,bound_owned,bound_neutral", [(256, 5e-13, 5e-13), (512, 3e-12, 8e-13), (1024, None, 2e-12)])
+def test_slope_path_rounding_vs_lattice_extent(torch_cuda, monkeypatch, Nk, bound_owned, bound_neutral):
+    """The table of DESIGN.md section 8, reproducibly: rounding error of the slope path in lattice mode against the
+    long-double oracle on the paper's AMR(3, D22) quadtrees (48 seeded targets), with owned per-patch weights (the
+    default up to a lattice extent of 4,096 units = N_k 512 here; measured 1.4e-13, 8.9e-13) and with own-cell
+    ("neutral") weights (the default beyond, forced by SG_LATTICE_NEUTRAL_WEIGHTS below; measured 9.2e-14, 1.5e-13,
+    3.9e-13).  The bounds leave a factor ~3-5 over the measured values; all are far inside the 1e-11 gate."""
+    from paper_2001_02765_b200 import SgDisk
+    lay = paper_ilr_layout(Nk, 3, "D22")
+    x, y, _ = cell_centres(lay)
+    sig, (sx, sy) = d22_sigma(x, y), d22_slopes(x, y)
+    idx = np.sort(np.random.default_rng(1).choice(lay.n_cells, 48, replace=False))
+    r = cell_rects(lay)
+    ox, oy, _ = oracle.force(r, sig, r["kxc"][idx], r["kyc"][idx], lay.unit, dx=sx, dy=sy)
+
+    def run():
+        with SgDisk.from_layout(lay, device=0) as d:
+            d.set_interaction_mode("lattice")
+            d.set_density_linear(*[torch_cuda.as_tensor(a).cuda() for a in (sig, sx, sy)])
+            Fx, Fy = d.force()
+            torch_cuda.cuda.synchronize()
+            return errors(Fx.cpu().numpy()[idx], Fy.cpu().numpy()[idx], ox, oy)[0]
+    if bound_owned is not None:                     # lattice extent <= 4,096: the default is the owned weights
+        assert run() <= bound_owned
+    monkeypatch.setenv("SG_LATTICE_NEUTRAL_WEIGHTS", "1")
+    assert run() <= bound_neutral
