@@ -30,7 +30,7 @@ struct LatticeArrays {
     double2 *fn = nullptr;            // the function lattices
     int64_t fn_entries = 0;           // entries per plane (sum over (level, class))
     double *wS = nullptr;             // [3][n_patches * kPatchQStride] per-patch weights of the slope path: -W0, a, c
-    bool lin_neutral = false;         // wS holds own-cell weights on all 17 x 17 vertices (sg_api.cu: slope_weights_neutral)
+    bool lin_neutral = false;         // wS holds own-cell weights on all 17 x 17 vertices (sg_api.cu: neutral_weights)
 };
 
 constexpr int kFnPlanesLin = 3;
