@@ -5,4 +5,4 @@ the path runs in the CUDA kernels of csrc/).  There is no CPU fallback: if libsg
 the import of :mod:`.binding` fails loudly.
 """
 from .binding import (SgDisk, SgError, lib_path, load_library, measure_fp64_peak, measure_fp64_mma_peak, version,  # noqa: F401
-                      shard_range, EXPORTED_SYMBOLS)
+                      shard_range, EXPORTED_SYMBOLS, force_uniform_static)

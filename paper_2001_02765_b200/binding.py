@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = (
     "sg_create", "sg_destroy", "sg_num_cells", "sg_num_vertices", "sg_layout_info", "sg_cell_geometry",
     "sg_set_density", "sg_set_density_linear", "sg_force", "sg_set_target_range", "sg_set_interaction_mode", "sg_lattice_plan_check", "sg_lattice_plan_fill", "sg_launch_counts", "sg_set_kernel_timing", "sg_get_kernel_times",
     "sg_kernel_model", "sg_kernel_instruction_counts", "sg_measure_fp64_peak", "sg_measure_fp64_mma_peak", "sg_last_error", "sg_version",
+    "sg_force_uniform_static", "sg_static_last_error",
 )
 
 
@@ -99,6 +100,10 @@ def load_library():
     lib.sg_last_error.argtypes = [vp]
     lib.sg_version.restype = ctypes.c_char_p
     lib.sg_version.argtypes = []
+    lib.sg_force_uniform_static.restype = c_int
+    lib.sg_force_uniform_static.argtypes = [c_int, c_int, c_dbl, vp, vp, vp, c_int, vp]
+    lib.sg_static_last_error.restype = ctypes.c_char_p
+    lib.sg_static_last_error.argtypes = []
     _lib = lib
     return lib
 
@@ -143,6 +148,44 @@ from .sharding import shard_range  # noqa: E402,F401  (re-exported: one definiti
 def _stream_ptr(device: int):
     import torch
     return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+STATIC_MAX_VERTICES, STATIC_MAX_SIDE = 66049, 1024     # SG_STATIC_MAX_VERTICES, SG_STATIC_MAX_SIDE of sg_disk_static.h
+
+
+def force_uniform_static(sigma, G=1.0, Fx=None, Fy=None):
+    """sg_force_uniform_static (include/sg_disk_static.h): Fx, Fy of the zeroth-order sum on one uniform grid, for
+    callers that cannot let the library allocate device memory (an application arena that owns the GPU, a time-step
+    loop that must not take cudaMalloc's device-wide synchronisation, a plug-in under a no-allocation rule).
+
+    sigma: CUDA float64 tensor [ny, nx] (x fastest), at most 256 x 256 cells ((nx+1)*(ny+1) <= 66,049).  Fx, Fy:
+    tensors of the same shape to write into; a caller that really cannot allocate passes both (they are created with
+    torch.empty only when left out, which is this binding's convenience, not the library's doing).  The library call
+    allocates nothing: the vertex weights go to a fixed array inside libsg_disk.so that every call on the device
+    shares, so calls that can overlap on the GPU (different streams, no event between them) race; calls on one stream
+    are safe.  The first call on a device also looks up that array's address: make it before any stream capture.
+    Asynchronous on torch's current stream of sigma's device."""
+    import torch
+    lib = load_library()
+    if not (isinstance(sigma, torch.Tensor) and sigma.is_cuda and sigma.dtype == torch.float64 and sigma.dim() == 2
+            and sigma.is_contiguous()):
+        raise SgError(SG_ERR_ARG, "sigma must be a contiguous CUDA float64 tensor [ny, nx]")
+    ny, nx = sigma.shape
+    dev = sigma.device.index
+    if Fx is None:
+        Fx = torch.empty_like(sigma)
+    if Fy is None:
+        Fy = torch.empty_like(sigma)
+    for t, name in ((Fx, "Fx"), (Fy, "Fy")):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.shape == sigma.shape and t.device == sigma.device):
+            raise SgError(SG_ERR_ARG, f"{name} must be a contiguous CUDA float64 tensor shaped like sigma, on its device")
+    rc = lib.sg_force_uniform_static(int(nx), int(ny), float(G), ctypes.c_void_p(sigma.data_ptr()),
+                                     ctypes.c_void_p(Fx.data_ptr()), ctypes.c_void_p(Fy.data_ptr()), int(dev),
+                                     _stream_ptr(dev))
+    if rc != SG_OK:
+        raise SgError(rc, lib.sg_static_last_error().decode())
+    return Fx, Fy
 
 
 class SgDisk:

@@ -7,8 +7,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsg_disk.so")
-SOURCES = ["sg_layout.cpp", "sg_kernels.cu", "sg_kernels_lin.cu", "sg_kernels_patch.cu", "sg_kernels_lattice.cu", "sg_api.cu"]
-HEADERS = ["sg_layout.h", "sg_kernels.cuh", "sg_device.cuh", "sg_kernels_lin.cuh", "sg_kernels_patch.cuh", "sg_patch_device.cuh", "sg_kernels_lattice.cuh", os.path.join("..", "..", "include", "sg_disk.h"), os.path.join("..", "..", "include", "sg_disk_diag.h")]
+SOURCES = ["sg_layout.cpp", "sg_kernels.cu", "sg_kernels_lin.cu", "sg_kernels_patch.cu", "sg_kernels_lattice.cu", "sg_api.cu", "sg_static.cu"]
+HEADERS = ["sg_layout.h", "sg_kernels.cuh", "sg_device.cuh", "sg_kernels_lin.cuh", "sg_kernels_patch.cuh", "sg_patch_device.cuh", "sg_kernels_lattice.cuh", os.path.join("..", "..", "include", "sg_disk.h"), os.path.join("..", "..", "include", "sg_disk_diag.h"), os.path.join("..", "..", "include", "sg_disk_static.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O3", "-Xcompiler", "-fopenmp", "--shared", "-cudart", "shared", "-lgomp"]
 
