@@ -116,7 +116,8 @@ int sg_set_density_linear(sg_ctx *ctx, const double *sigma_dev, const double *dx
  * Test aid: with the environment variable SG_POISON_PARTIALS set, the internal partial-sum buffer is filled
  * with NaN on cuda_stream at the start of every sg_force, so that a partial sum no kernel wrote surfaces in Fx, Fy.
  * Debugging aid: with SG_DEBUG_SYNC set, lattice mode synchronises after every pair-class launch and names the one
- * that failed in sg_last_error (it serialises the launches; not for timing).
+ * that failed in sg_last_error (it serialises the launches; not for timing).  Both variables are read once, at
+ * sg_create; sg_force itself reads no environment.
  */
 int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
 
@@ -149,9 +150,12 @@ int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
  *   SG_MODE_LATTICE_BLOCKED  as SG_MODE_LATTICE, but SG_ERR_ARG unless P = 16.  For tests and profiling.
  *   SG_MODE_LATTICE_INCTA    P = 16, offset tables built inside the CTAs at every sg_force (the round-1 kernels; no
  *                    table memory; zeroth-order path only).  Bit-identical to SG_MODE_LATTICE.
- * Environment, read at sg_create: SG_LATTICE_NEUTRAL_WEIGHTS selects per-patch weights from the patch's own cells on all
- * 17 x 17 vertices (every patch neutral: less rounding on steep, deep hierarchies, 7 % slower) instead of deduplicated
- * weights owned on 16 x 16 vertices; same sum.
+ * Per-patch weights of lattice mode (same sum either way): the zeroth-order path uses deduplicated weights owned on
+ * 16 x 16 vertices of a patch on lattices of up to 4,096 units (extent / (h_fin / 2)), and weights from the patch's own
+ * cells on all 17 x 17 vertices (every patch neutral: less rounding on steep, deep hierarchies, 7-8 % slower) beyond
+ * -- the library switches by itself -- or everywhere when SG_LATTICE_NEUTRAL_WEIGHTS is set (read at sg_create).  The
+ * slope path always uses the neutral weights: its planes enter multiplied by the lattice offset, and only neutral
+ * patches keep it at the accuracy of the direct slope kernel (BASELINE config 4: rel. L2 1.7e-12 owned, gate 1e-12).
  * Host-synchronous: may allocate and build tables; not to be called during stream capture.
  */
 #define SG_MODE_DIRECT  0

@@ -34,6 +34,10 @@ struct sg_ctx {
     int patch_n_groups[3] = {0, 0, 0};      // sizes of the three group lists (offset_group_list)
     bool use_patch = false;      // sg_set_interaction_mode
     bool neutral_weights = false; // SG_LATTICE_NEUTRAL_WEIGHTS at sg_create: own-cell per-patch weights (sg_kernels_patch.cu)
+    // environment switches, latched at sg_create (sg_force reads no environment)
+    bool poison_partials = false;     // SG_POISON_PARTIALS: NaN-fill the partial sums before every sg_force (test aid)
+    bool debug_sync = false;          // SG_DEBUG_SYNC: synchronise after every pair-class launch (debugging aid)
+    bool owned_slope_weights = false; // SG_LATTICE_OWNED_SLOPE_WEIGHTS: round-2 owned weights on the lattice slope path
     bool force_incta = false;    // SG_MODE_LATTICE_INCTA: offset tables built inside the CTAs even if the lattices exist
     LatticeArrays lat;           // precomputed function lattices of the pair classes (sg_kernels_lattice.cu)
     std::vector<FnLattice> lat_meta;        // host copy, [n_levels * kOffClasses]
@@ -42,6 +46,8 @@ struct sg_ctx {
     // 16 x 16 blocks of an inner context that runs the lattice kernels; cell data is permuted in and out
     sg_ctx *inner = nullptr;
     int32_t *rg_map = nullptr, *rg_inv = nullptr;       // device: caller cell -> inner cell; inner cell -> caller cell or -1
+    std::vector<int32_t> rg_map_host;                   // host copy of rg_map (sg_set_target_range -> inner block range)
+    int64_t rg_first = 0;                               // first inner cell of the inner context's target range
     double *rg_in[3] = {nullptr, nullptr, nullptr};     // sigma, dx, dy in inner cell order
     double *rg_f[2] = {nullptr, nullptr};               // Fx, Fy in inner cell order
     int64_t first = 0, count = 0;
@@ -256,29 +262,40 @@ int64_t plan_fn_lattices(sg_ctx *c) {
 }
 
 // Memory budget of the function lattices (all planes): SG_LATTICE_TABLE_MIB, default a quarter of the device's memory
-// (45 GB on a B200).  Over it, lattice mode builds its offset tables inside the CTAs (patch_offset_kernel) and the
-// slope path stays direct.
+// (45 GB on a B200) or what is free right now, whichever is less.  Over it, lattice mode builds its offset tables
+// inside the CTAs (patch_offset_kernel) and the slope path stays direct.
 int64_t fn_budget_bytes() {
     if (const char *e = std::getenv("SG_LATTICE_TABLE_MIB")) return std::max<int64_t>(0, std::atoll(e)) << 20;
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return int64_t(16) << 30;
-    return int64_t(total_b / 4);
+    return int64_t(std::min(free_b, total_b / 4));
 }
 
 // Build (or extend to the slope planes) the function lattices.  Host-synchronous; no-op when they exist already.
+// Never fails for lack of memory: over the budget, or when the allocation itself fails, whatever lattice exists stays
+// in place (a 1-plane lattice keeps serving the zeroth-order path) and the caller's path falls back as sg_disk.h says
+// (in-CTA tables / direct slope kernel).  The new buffer is allocated BEFORE the old one is released.
 int ensure_fn_lattices(sg_ctx *c, int n_planes) {
     if (c->device < 0 || !c->patch.blocked || c->lat_entries == 0) return SG_OK;
     if (c->lat.n_planes_built >= n_planes) return SG_OK;
-    if (c->lat_entries * 16 * n_planes > fn_budget_bytes()) return SG_OK;      // stays on the in-CTA tables
+    const int64_t need = c->lat_entries * 16 * n_planes;
+    if (need > fn_budget_bytes()) return SG_OK;                                // stays on the fallback
     SG_CUDA(c, cudaDeviceSynchronize());
+    void *fresh = nullptr;
+    if (cudaMalloc(&fresh, size_t(need)) != cudaSuccess) {
+        cudaGetLastError();                                                    // not sticky: clear it, keep what exists
+        return SG_OK;
+    }
     if (c->lat.fn) {
         cudaFree(c->lat.fn);
         c->allocs.erase(std::remove(c->allocs.begin(), c->allocs.end(), (void *)c->lat.fn), c->allocs.end());
         c->dev_bytes -= c->lat_entries * 16 * c->lat.n_planes_built;
-        c->lat.fn = nullptr; c->lat.n_planes_built = 0; c->lat.ready = false;
+        c->lat.n_planes_built = 0; c->lat.ready = false;
     }
-    int rc = dev_alloc(c, &c->lat.fn, c->lat_entries * n_planes);
-    if (rc) return rc;
+    c->lat.fn = static_cast<decltype(c->lat.fn)>(fresh);
+    c->allocs.push_back(fresh);
+    c->dev_bytes += need;
+    int rc;
     for (FnLattice &m : c->lat_meta) m.plane_stride = c->lat_entries;
     if (!c->lat.meta) {
         if ((rc = upload(c, &c->lat.meta, c->lat_meta))) return rc;
@@ -643,6 +660,9 @@ static int create_ctx(sg_ctx **out, int n_levels, const double *cell_width, doub
         c->device = device;
         c->dev.G = G;
         c->first = 0; c->count = c->host.N;
+        c->poison_partials = std::getenv("SG_POISON_PARTIALS") != nullptr;
+        c->debug_sync = std::getenv("SG_DEBUG_SYNC") != nullptr;
+        c->owned_slope_weights = std::getenv("SG_LATTICE_OWNED_SLOPE_WEIGHTS") != nullptr;
         c->patch_plan_ok = build_patch_plan(c);
         c->lat_entries = plan_fn_lattices(c);
         if (device >= 0) {
@@ -671,6 +691,8 @@ int sg_create(sg_ctx **out, int n_levels, const double *cell_width, double x0, d
               const sg_patch *leaf_patches, int64_t n_patches, double G, int device) {
     return create_ctx(out, n_levels, cell_width, x0, y0, patch_cells, leaf_patches, n_patches, G, device, nullptr);
 }
+
+static int apply_inner_range(sg_ctx *c);
 
 // Regrouping for lattice mode (P = 1, 2, 4): every leaf cell of level l at (ci, cj) on its level's lattice goes to
 // the aligned 16 x 16 block (l, ci >> 4, cj >> 4); a block that is only partly covered by leaves of its level is
@@ -718,13 +740,44 @@ static int build_regrouped(sg_ctx *c) {
     sg_ctx *in = nullptr;
     int rc = create_ctx(&in, h.n_levels, cw.data(), h.x0, h.y0, 16, bp.data(), nb, c->dev.G, c->device, present.data());
     if (rc != SG_OK) { c->err = "regrouped layout: " + g_create_error; return rc; }
+    // c->inner is what marks the regrouping as built (sg_set_interaction_mode, sg_set_density, sg_force): it is set
+    // only once every permutation buffer exists; on a failure the inner context goes and a later call starts over
+    // (buffers already allocated stay owned by c and are freed by sg_destroy)
+    rc = upload(c, &c->rg_map, map);
+    if (rc == SG_OK) rc = upload(c, &c->rg_inv, inv);
+    for (int k = 0; k < 3 && rc == SG_OK; ++k) rc = dev_alloc(c, &c->rg_in[k], n_inner);
+    for (int k = 0; k < 2 && rc == SG_OK; ++k) rc = dev_alloc(c, &c->rg_f[k], n_inner);
+    if (rc != SG_OK) {
+        sg_destroy(in);
+        c->rg_map = c->rg_inv = nullptr;
+        for (double *&q : c->rg_in) q = nullptr;
+        for (double *&q : c->rg_f) q = nullptr;
+        return rc;
+    }
     c->inner = in;
-    if ((rc = upload(c, &c->rg_map, map)) || (rc = upload(c, &c->rg_inv, inv))) return rc;
-    for (int k = 0; k < 3; ++k)
-        if ((rc = dev_alloc(c, &c->rg_in[k], n_inner))) return rc;
-    for (int k = 0; k < 2; ++k)
-        if ((rc = dev_alloc(c, &c->rg_f[k], n_inner))) return rc;
-    return SG_OK;
+    c->rg_map_host = std::move(map);
+    return apply_inner_range(c);                                  // a target range set before the mode was chosen
+}
+
+// Regrouped lattice mode: a target slice must cost a slice (targets are shared out over GPUs).  The
+// caller's range [first, first + count) is turned into the range of inner blocks that hold its cells, and the inner
+// context evaluates only those: the caller's cell order (level, row, column) and the block order (level, block row,
+// block column) run alike when the patch list is sorted that way (the usual case; any order is still correct, the
+// covering range just grows), so the covering block range exceeds the slice by about two block rows per level touched.  rg_first is the inner cell the slice-relative rg_f buffers start at (gather_cells_kernel subtracts it).
+static int apply_inner_range(sg_ctx *c) {
+    if (!c->inner) return SG_OK;
+    int64_t f = 0, n = 0;
+    if (c->count > 0) {
+        int32_t kmin = INT32_MAX, kmax = -1;
+        const int32_t *m = c->rg_map_host.data() + c->first;
+        for (int64_t i = 0; i < c->count; ++i) { kmin = std::min(kmin, m[i]); kmax = std::max(kmax, m[i]); }
+        f = int64_t(kmin / 256) * 256;
+        n = (int64_t(kmax / 256) + 1) * 256 - f;
+    }
+    c->rg_first = f;
+    const int rc = sg_set_target_range(c->inner, f, n);
+    if (rc) c->err = c->inner->err;
+    return rc;
 }
 
 static bool regroupable(const sg_ctx *c) { return c->host.P == 1 || c->host.P == 2 || c->host.P == 4; }
@@ -819,15 +872,22 @@ int sg_set_density_linear(sg_ctx *c, const double *sigma_dev, const double *dx_d
         SG_CUDA(c, configure_lin_kernels(d.tab_entries));
         if (c->patch.blocked && (rc = dev_alloc(c, &c->lat.wS, int64_t(kFnPlanesLin) * c->patch.n_patches * kPatchQStride)))
             return rc;
-        l.allocated = true;
         // lattice mode is on already: add the slope planes to the function lattices (host-synchronous, first call only)
         if (c->use_patch && !c->force_incta && (rc = ensure_fn_lattices(c, kFnPlanesLin))) return rc;
         if ((rc = reserve_partials(c))) return rc;
+        l.allocated = true;                                       // only now: a failed set-up is retried by the next call
     }
     launch_weights_lin(c->dev, l, sigma_dev, dx_dev, dy_dev, s);
     if (c->lat.wS) {
-        // slope path in lattice mode: the same choice of per-patch weights as the zeroth-order path (upload_patches)
-        c->lat.lin_neutral = c->neutral_weights;
+        // slope path in lattice mode: ALWAYS own-cell (neutral) per-patch weights on all 17 x 17 vertices.  The slope
+        // planes a_v, c_v enter multiplied by the lattice offset u, v, so owned 16 x 16 weights (patches not neutral)
+        // cancel across patches and lose digits with extent / h: BASELINE config 4 (extent 2,048) rel. L2 1.7e-12
+        // owned against 7e-13 with the direct slope kernel and the 1e-12 gate; neutral weights are as accurate as the
+        // direct kernel at every extent.  Costs 289 instead of 256 vertices per patch pair on this path
+        // only; the zeroth-order path keeps the choice made in upload_patches.  SG_LATTICE_OWNED_SLOPE_WEIGHTS (read at
+        // sg_create) brings the owned weights back on lattices of up to 4,096 units: a test aid that reproduces the
+        // comparison table of DESIGN.md 8, not a supported mode.
+        c->lat.lin_neutral = c->neutral_weights || !c->owned_slope_weights;
         if (c->lat.lin_neutral) launch_patch_weights_lin_owncell(c->patch, sigma_dev, dx_dev, dy_dev, l.patch_hh, l.unit, c->lat.wS, s);
         else launch_patch_weights_lin(c->patch, l.wl, c->lat.wS, s);
     }
@@ -852,14 +912,15 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     DeviceGuard guard(c->device);
     SG_CUDA(c, guard.err);
     if (c->use_patch && c->inner) {
-        // regrouped lattice mode: the inner context evaluates every block, the caller's targets are picked out of it
+        // regrouped lattice mode: the inner context evaluates the blocks that hold the caller's target range
+        // (apply_inner_range), the caller's targets are picked out of its slice-relative result
         if (!c->inner->density_set || c->inner->linear != c->linear) {
             c->err = "regrouped lattice mode: set the density after sg_set_interaction_mode(SG_MODE_LATTICE)";
             return SG_ERR_STATE;
         }
         const int rc = sg_force(c->inner, c->rg_f[0], c->rg_f[1], cuda_stream);
         if (rc) { c->err = c->inner->err; return rc; }
-        launch_gather_cells(c->rg_f[0], c->rg_f[1], c->rg_map, c->first, c->count, Fx_dev, Fy_dev, s);
+        launch_gather_cells(c->rg_f[0], c->rg_f[1], c->rg_map, c->rg_first, c->first, c->count, Fx_dev, Fy_dev, s);
         SG_CUDA(c, cudaGetLastError());
         return SG_OK;
     }
@@ -869,7 +930,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
     if (rc) return rc;
     // test aid (tests/conftest.py sets it): NaN-fill the partial sums on the caller's stream before EVERY evaluation,
     // so that a slot no kernel writes shows up in the forces instead of passing as the previous call's value
-    if (std::getenv("SG_POISON_PARTIALS"))
+    if (c->poison_partials)
         SG_CUDA(c, cudaMemsetAsync(c->dev.part, 0xFF, size_t(sp.partials()) * sizeof(double), s));
     const int slot = int(c->timed_calls % kTimingRing);
     if (c->timing) SG_CUDA(c, cudaEventRecord(c->ev0[slot], s));
@@ -880,7 +941,7 @@ int sg_force(sg_ctx *c, double *Fx_dev, double *Fy_dev, void *cuda_stream) {
         // an event recorded on the caller's stream and are joined back into it (capturable in a CUDA graph)
         const OffsetPlan &po = sp.po;
         double *part = c->dev.part;
-        const bool debug_sync = std::getenv("SG_DEBUG_SYNC") != nullptr;   // debugging aid: name the failing launch
+        const bool debug_sync = c->debug_sync;                 // debugging aid: name the failing launch
         const int n_total = (sp.blocked ? offset_classes(po) : 0) + ((!sp.blocked || sp.far) ? 1 : 0);
         if (n_total > 1) {
             while (int(c->side.size()) < n_total - 1) {
@@ -1005,6 +1066,8 @@ int sg_set_target_range(sg_ctx *c, int64_t first, int64_t count) {
     if (c->device < 0) return SG_OK;
     DeviceGuard guard(c->device);
     SG_CUDA(c, guard.err);
+    const int rc = apply_inner_range(c);
+    if (rc) return rc;
     return reserve_partials(c);
 }
 
@@ -1104,20 +1167,8 @@ int sg_lattice_plan_fill(const sg_ctx *c, int64_t *out) {
     return SG_OK;
 }
 
-int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
-    if (!c) return SG_ERR_ARG;
-    if (c->inner) {                                               // + the permutation kernels
-        int a = 0, b = 0, a2 = 0, b2 = 0;
-        sg_launch_counts(c->inner, &a, &b);
-        sg_ctx *mut = const_cast<sg_ctx *>(c);                    // own counts as if there were no inner context
-        sg_ctx *saved = mut->inner;
-        mut->inner = nullptr;
-        sg_launch_counts(c, &a2, &b2);
-        mut->inner = saved;
-        if (set_density_launches) *set_density_launches = a2 + 1 + a;
-        if (force_launches) *force_launches = c->use_patch ? (c->count > 0 ? b + 1 : 0) : b2;
-        return SG_OK;
-    }
+// Launches of the context's OWN path (as if it had no inner context); read-only on the context.
+static void own_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
     // vertex weights, running sums and look-ups per direction (+ per-patch weights when the lattice-offset path exists);
     // with slopes: weights, column tables, row tables (+ per-patch slope weights)
     if (set_density_launches) *set_density_launches = c->linear ? 3 + (c->lat.wS ? 1 : 0) : 5 + (c->patch.enabled ? 1 : 0);
@@ -1129,6 +1180,19 @@ int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_laun
         }
         *force_launches = c->count > 0 ? n + 1 : 0;
     }
+}
+
+int sg_launch_counts(const sg_ctx *c, int *set_density_launches, int *force_launches) {
+    if (!c) return SG_ERR_ARG;
+    if (c->inner) {                                               // + the permutation kernels
+        int a = 0, b = 0, a2 = 0, b2 = 0;
+        sg_launch_counts(c->inner, &a, &b);
+        own_launch_counts(c, &a2, &b2);
+        if (set_density_launches) *set_density_launches = a2 + 1 + a;
+        if (force_launches) *force_launches = c->use_patch ? (c->count > 0 ? b + 1 : 0) : b2;
+        return SG_OK;
+    }
+    own_launch_counts(c, set_density_launches, force_launches);
     return SG_OK;
 }
 

@@ -357,11 +357,11 @@ __global__ void scatter_cells_kernel(const double *__restrict__ a, const double 
 }
 
 __global__ void gather_cells_kernel(const double *__restrict__ fx, const double *__restrict__ fy,
-                                    const int32_t *__restrict__ map, int64_t first, int64_t count,
+                                    const int32_t *__restrict__ map, int64_t base, int64_t first, int64_t count,
                                     double *__restrict__ ox, double *__restrict__ oy) {
     const int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= count) return;
-    const int32_t k = map[first + i];
+    const int64_t k = int64_t(map[first + i]) - base;   // fx, fy hold the inner target range, which starts at `base`
     ox[i] = fx[k];
     oy[i] = fy[k];
 }
@@ -371,9 +371,9 @@ void launch_scatter_cells(const double *a, const double *b, const double *c, con
     scatter_cells_kernel<<<unsigned((n_inner + 255) / 256), 256, 0, s>>>(a, b, c, inv, oa, ob, oc, n_inner);
 }
 
-void launch_gather_cells(const double *fx, const double *fy, const int32_t *map, int64_t first, int64_t count,
-                         double *ox, double *oy, cudaStream_t s) {
-    if (count > 0) gather_cells_kernel<<<unsigned((count + 255) / 256), 256, 0, s>>>(fx, fy, map, first, count, ox, oy);
+void launch_gather_cells(const double *fx, const double *fy, const int32_t *map, int64_t base, int64_t first,
+                         int64_t count, double *ox, double *oy, cudaStream_t s) {
+    if (count > 0) gather_cells_kernel<<<unsigned((count + 255) / 256), 256, 0, s>>>(fx, fy, map, base, first, count, ox, oy);
 }
 
 // ------------------------------------------------------------------------------------------------

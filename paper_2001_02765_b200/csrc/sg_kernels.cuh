@@ -97,8 +97,8 @@ cudaError_t measure_dmma(double *dmma_tflops, double *mixed_tflops);   // FP64 m
 // regrouped layouts: caller cell order <-> padded block order (b, c may be null: sigma only)
 void launch_scatter_cells(const double *a, const double *b, const double *c, const int32_t *inv, double *oa, double *ob,
                           double *oc, int64_t n_inner, cudaStream_t s);
-void launch_gather_cells(const double *fx, const double *fy, const int32_t *map, int64_t first, int64_t count,
-                         double *ox, double *oy, cudaStream_t s);
+void launch_gather_cells(const double *fx, const double *fy, const int32_t *map, int64_t base, int64_t first,
+                         int64_t count, double *ox, double *oy, cudaStream_t s);
 
 // FP64-pipe warp instructions and FLOPs per (target, vertex slot) of the interaction kernel as written
 // (cross-checked against cuobjdump -sass): per pair 16 DFMA + 3 DADD + 2 DMUL,

@@ -319,6 +319,48 @@ def test_regrouped_small_patches_vs_oracle(torch_cuda, name):
         assert np.array_equal(rx, gx[first:first + count]) and np.array_equal(ry, gy[first:first + count])
 
 
+def test_regrouped_rank_slices_cost_a_slice(torch_cuda):
+    """A target slice of a regrouped layout costs a slice (the paper shares targets out over 12 cards; its
+    quadtrees have 1-cell patches): on the paper's ILR quadtree (N_k = 256, three levels) the cost-balanced slices of
+    three "ranks", run one after another on this device, concatenate bit-identically to the unsharded result, and the
+    interaction kernels of every slice take at most 0.45 of the full evaluation's time (a third each, plus the block
+    rows at the cuts and the launch tails).  The range may be set before or after the mode is chosen."""
+    from paper_2001_02765_b200 import SgDisk
+    from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
+    lay = paper_ilr_layout(256, 3)
+    sigma = torch_cuda.as_tensor(_noisy_kuzmin(lay, 92)).cuda()
+    costs = lattice_patch_costs(lay.patches[:, 0])
+    world = 3
+
+    def timed(d):
+        d.set_density(sigma)
+        d.force()                                                  # warm-up
+        d.set_kernel_timing(True)
+        out = [d.force() for _ in range(3)][-1]
+        torch_cuda.cuda.synchronize()
+        ms = min(d.kernel_times_ms())
+        d.set_kernel_timing(False)
+        return out[0].cpu().numpy(), out[1].cpu().numpy(), ms
+
+    with SgDisk.from_layout(lay, device=0) as d:
+        d.set_interaction_mode("lattice")
+        fx, fy, ms_full = timed(d)
+        px, py, ms_slices = [], [], []
+        for r in range(world):
+            d.set_target_range(*shard_range_by_cost(costs, lay.P * lay.P, r, world))
+            gx, gy, ms = timed(d)
+            px.append(gx); py.append(gy); ms_slices.append(ms)
+    assert np.array_equal(np.concatenate(px), fx) and np.array_equal(np.concatenate(py), fy)
+    assert max(ms_slices) <= 0.45 * ms_full, (ms_slices, ms_full)
+    with SgDisk.from_layout(lay, device=0) as d:                   # range first, mode second
+        first, count = shard_range_by_cost(costs, lay.P * lay.P, 1, world)
+        d.set_target_range(first, count)
+        d.set_interaction_mode("lattice")
+        d.set_density(sigma)
+        gx, gy = [t.cpu().numpy() for t in d.force()]
+    assert np.array_equal(gx, px[1]) and np.array_equal(gy, py[1])
+
+
 def test_regrouped_mode_state_and_mode_switches(torch_cuda):
     """Density set before lattice mode was selected on a small-patch layout: sg_force refuses (SG_ERR_STATE) instead of
     using a stale inner density; after set_density both modes work on one context, any order."""
