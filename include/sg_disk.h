@@ -126,6 +126,11 @@ int sg_force(sg_ctx *ctx, double *Fx_dev, double *Fy_dev, void *cuda_stream);
  * still summed).  Fx_dev/Fy_dev then hold count values.  This is how the path shards over GPUs:
  * targets are independent, each rank owns a slice, no collective is needed.
  * count == 0 is allowed (sg_force does nothing).  Default: first = 0, count = N.
+ * The cost follows the slice in every mode; a regrouped layout (P = 1, 2, 4 in SG_MODE_LATTICE) evaluates the 16 x 16
+ * blocks that hold the slice (the covering block range: tight when the patch list is sorted by level, row, column).
+ * In the lattice modes a slice is bit-identical to the same targets of the full evaluation (the source lists are split
+ * as for the full range); in SG_MODE_DIRECT the source split depends on the range and a slice agrees with the full
+ * evaluation to rounding (1e-13 of max|F|).
  */
 int sg_set_target_range(sg_ctx *ctx, int64_t first, int64_t count);
 

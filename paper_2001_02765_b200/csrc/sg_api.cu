@@ -174,7 +174,9 @@ PatchPlan make_patch_plan(const sg_ctx *c) {
     pp.first_patch = int(c->first / PP);
     pp.n_tpatches = int((c->first + c->count - 1) / PP) - pp.first_patch + 1;
     const int slots = c->sm_count * (pa.P == 16 ? 2 : 4);
-    int want = (8 * slots + pp.n_tpatches - 1) / pp.n_tpatches;            // about 8 items per resident CTA
+    // The split of the source list is that of the FULL evaluation whatever the target range: a slice then adds the
+    // same partial sums in the same order as the unsharded call, so rank slices are bit-identical to it.
+    int want = (8 * slots + pa.n_patches - 1) / std::max(1, pa.n_patches);  // about 8 items per resident CTA (full range)
     want = std::max(1, std::min(want, std::max(1, pa.n_patches / 4)));     // but >= 4 source patches per item
     pp.patches_per_split = (pa.n_patches + want - 1) / want;
     pp.n_split = (pa.n_patches + pp.patches_per_split - 1) / pp.patches_per_split;
@@ -196,20 +198,27 @@ OffsetPlan make_offset_plan(const sg_ctx *c, const PatchPlan &pp) {
     for (int q = 0; q < 3; ++q) po.n_groups[q] = c->patch_n_groups[q];
     po.first_patch = pp.first_patch;
     po.last_patch = pp.first_patch + pp.n_tpatches - 1;
-    int touched = 0;
+    bool any[kOffClasses] = {false, false, false, false, false};
     for (size_t i = 0; i < c->patch_groups.size(); ++i) {
         const PatchGroup &g = c->patch_groups[i];
+        for (int v = 0; v < kOffClasses; ++v) any[v] = any[v] || g.box[v][1] > 0;
         if (g.pmax < po.first_patch || g.pmin > po.last_patch) continue;
-        if (int(i) < po.n_groups[0]) ++touched;
         for (int v = 0; v < kOffClasses; ++v) po.variant[v] = po.variant[v] || g.box[v][1] > 0;
     }
+    // n_split is chosen for the FULL evaluation (all groups, all N targets) whatever the target range: every group's
+    // offset list is then cut the same way in a slice as in the unsharded call and the partial sums are added in the
+    // same order, so rank slices (sg_set_target_range, regrouped layouts included) are bit-identical to it.  A rank
+    // of an N-GPU run gets 1/N of the ~16 items per resident CTA.
+    const int touched = po.n_groups[0];
+    int64_t classes = 0;
+    for (int v = 0; v < kOffClasses; ++v) classes += any[v] ? 1 : 0;
+    classes = std::max<int64_t>(1, classes);
     // splits of every group's offset list: about 16 work items per resident CTA (items of sparse levels differ a lot in
     // weight; the queue is dynamic), and among the next few counts the one whose item count fills the last wave of the
     // persistent grid best (on a uniform level all items weigh the same: 512 groups x 4 splits ran 13 % faster than
     // x 3, and x 6 slower than x 4)
     const int slots = c->sm_count * 2;
-    const int64_t classes = std::max(1, offset_classes(po));
-    const int64_t mem_cap = std::max<int64_t>(1, (int64_t(1) << 30) / (classes * 16 * std::max<int64_t>(1, c->count)));
+    const int64_t mem_cap = std::max<int64_t>(1, (int64_t(1) << 30) / (classes * 16 * std::max<int64_t>(1, c->host.N)));
     const int cap = int(std::min<int64_t>(64, mem_cap));              // partial sums stay below 1 GiB
     const int want = std::max(1, std::min(cap, (16 * slots + touched - 1) / std::max(1, touched)));
     double best = -1.0;
