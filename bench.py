@@ -269,7 +269,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2001_02765_b200 import SgDisk, measure_fp64_peak, measure_fp64_mma_peak, shard_range
-    from paper_2001_02765_b200.sharding import lattice_patch_costs, shard_range_by_cost
+    from paper_2001_02765_b200.sharding import lattice_patch_costs, regrouped_patch_costs, shard_range_by_cost
     from workloads import make_config, expected_counts
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -296,7 +296,8 @@ def run_ours(args):
         # lattice mode works on whole patches and a target's cost depends on its level: split by estimated cost
         # (small patches are regrouped into 16 x 16 blocks inside the library, which evaluates the blocks that hold
         # the slice: the same per-level estimate applies)
-        first, count = shard_range_by_cost(lattice_patch_costs(lay.patches[:, 0]), lay.P * lay.P, rank, world)
+        costs = (lattice_patch_costs(lay.patches[:, 0]) if lay.P == 16 else regrouped_patch_costs(lay.patches, lay.P))
+        first, count = shard_range_by_cost(costs, lay.P * lay.P, rank, world)
     else:
         first, count = shard_range(N, rank, world)
 

@@ -127,7 +127,9 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     double2 *ring = reinterpret_cast<double2 *>(smem_raw);                 // [K][TBUF]
     int *sB = reinterpret_cast<int *>(ring + K * TBUF);                    // [kChunkOffsets][8]
     int *sLive = sB + kChunkOffsets * 8;                                   // [kChunkOffsets]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sLive + kChunkOffsets);  // [8]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sLive + kChunkOffsets);  // [4] "full": the stage's TMA bytes have landed
+    uint64_t *empty = full + 4;                                            // [4] "empty": all 8 warps are done reading it
+    static_assert(K <= 4, "full[] and empty[] share eight mbarrier slots");
     int *sDone = reinterpret_cast<int *>(full + 8);                        // [8]
     int *sPos = sDone + 8;                                                 // [8][2] patch position of target patch w
     int *sMisc = sPos + 16;                                                // [0] item, [1] live offsets of the chunk
@@ -135,7 +137,7 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
     const int l = lane & 15, h = lane >> 4;
 
     if (tid == 0) {
-        for (int k = 0; k < K; ++k) { mbar_init(&full[k], 1); sDone[k] = 0; }
+        for (int k = 0; k < K; ++k) { mbar_init(&full[k], 1); mbar_init(&empty[k], kOffWarps); sDone[k] = 0; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     uint32_t gs = 0;                  // stages this CTA has been through (the same in every warp): slot and parity
@@ -175,8 +177,13 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
             const int dx = dpi_min + STEP * (n % ndpi), dy = dpj_min + STEP * (n / ndpi);
             const double2 *src = fn + fm.base + int64_t(pl) * fm.plane_stride +
                                  int64_t(P * dy - fm.rmin) * fm.ncols + (P * dx - fm.cmin);
-            const uint32_t slot = (gs + uint32_t(s)) % K;
+            const uint32_t g = gs + uint32_t(s), slot = g % K;
             const int nrows = V == kOffCoarserSrc4 ? (sub < 4 ? 28 : 16) : LatCls<V>::SLOT_ROWS;
+            // Producer acquire: the slot's previous use (stage g - K) was read through the generic proxy by all eight
+            // warps, each of which arrived on empty[slot] afterwards; the TMA writes below go through the async proxy
+            // and are issued only after that phase has completed -- the mbarrier empty / full protocol, for the
+            // refills inside a chunk and for the first K stages of a chunk alike.
+            if (g >= uint32_t(K)) mbar_wait(&empty[slot], ((g / K) - 1u) & 1u);
             if (lane == 0) mbar_expect_tx(&full[slot], uint32_t(nrows) * TROW * 16);
             __syncwarp();
             for (int r = lane; r < nrows; r += 32) {
@@ -237,6 +244,7 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
             __syncthreads();
             const int S = sMisc[1] * n_planes * NSUB;                     // stages of this chunk
             // (3) the ring: warp 0 fills the first K stages, afterwards the last warp to release a stage refills it
+            // (full[slot]: TMA complete_tx -> consumers; empty[slot]: 8 consumer arrivals -> the issuing warp)
             if (warp == 0)
                 for (int s = 0; s < min(K, S); ++s) issue_stage(s, cb);
             for (int s = 0; s < S; ++s) {
@@ -247,8 +255,12 @@ lattice_corr_kernel(const PatchInfo *__restrict__ info, const PatchLevel *__rest
                 mbar_wait(&full[slot], (g / K) & 1u);                     // also for a warp without work: a warp
                 if (my_patch >= 0 && b >= 0) consume(b, pl, sub, ring + slot * TBUF);   // never runs more than K stages ahead
                 __syncwarp();
+                // Consumer release: every warp arrives on empty[slot] (this is what orders its reads of the stage before
+                // the refill, see issue_stage).  The counter only ELECTS the refilling warp -- the one that arrived last,
+                // so that no warp waits for a slower one here; its wait on empty[slot] returns at once.
                 int last = 0;
                 if (lane == 0) {
+                    mbar_arrive(&empty[slot]);
                     __threadfence_block();
                     last = atomicAdd(&sDone[slot], 1) == kOffWarps - 1;
                     if (last) atomicExch(&sDone[slot], 0);

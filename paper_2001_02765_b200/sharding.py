@@ -35,10 +35,41 @@ def lattice_patch_costs(patch_levels, far_weight: float = 10.5, near_levels: int
     return [cost_of_level[l] for l in levels]
 
 
+def regrouped_patch_costs(patches, patch_cells: int, far_weight: float = 10.5, near_levels: int = 2):
+    """Estimated lattice-mode cost of every leaf patch of a layout of small patches (1, 2 or 4 cells a side, e.g. the
+    paper's zone-wise quadtrees), which the library regroups into padded 16 x 16 blocks: the kernels work on whole
+    blocks, holes included, so a block of level l costs sum_m n_blocks(m) * (1 or ``far_weight``) whatever its fill,
+    and every patch in it carries an equal share.  A patch of a sparsely filled block (the rim of a refined region)
+    is therefore dearer than one of a full block.
+
+    ``patches``: integer array [n, 3] = (level, i0, j0) in library patch order; returns a float array [n] for
+    ``shard_range_by_cost``.  (numpy: these layouts have millions of patches.)"""
+    import numpy as np
+    pa = np.asarray(patches, dtype=np.int64).reshape(-1, 3)
+    if patch_cells not in (1, 2, 4):
+        raise ValueError("regrouped_patch_costs is for patches of 1, 2 or 4 cells a side")
+    # a patch is aligned to its own size, which divides 16: all its cells fall into one block
+    key = (pa[:, 0] << 56) | ((pa[:, 2] >> 4) << 28) | (pa[:, 1] >> 4)
+    blocks, inverse, per_block = np.unique(key, return_inverse=True, return_counts=True)
+    n_levels = int(pa[:, 0].max()) + 1
+    blocks_of_level = np.bincount(blocks >> 56, minlength=n_levels).astype(np.float64)
+    dist = np.abs(np.arange(n_levels)[:, None] - np.arange(n_levels)[None, :])
+    cost_of_level = (np.where(dist <= near_levels, 1.0, far_weight) * blocks_of_level[None, :]).sum(axis=1)
+    return cost_of_level[pa[:, 0]] / per_block[inverse]
+
+
 def shard_range_by_cost(patch_costs, cells_per_patch: int, rank: int, world: int):
     """Contiguous target slice [first, first+count) of rank ``rank``, cut at patch boundaries so that the cumulative
     cost is split as evenly as whole patches allow.  The slices of ranks 0..world-1 partition [0, N)."""
     n = len(patch_costs)
+    if n > 100000:                                     # millions of 1-cell patches: the same cuts by prefix sums
+        import numpy as np
+        c = np.asarray(patch_costs, dtype=np.float64)
+        mid = np.cumsum(c) - 0.5 * c                   # patch p goes left of cut r iff its midpoint <= total r / world
+        total = float(c.sum())
+        cuts = [0] + [int(np.searchsorted(mid, total * r / world, side="right")) for r in range(1, world)] + [n]
+        first, last = cuts[rank], cuts[rank + 1]
+        return first * cells_per_patch, (last - first) * cells_per_patch
     total = float(sum(patch_costs))
     cuts = [0]
     acc, p = 0.0, 0

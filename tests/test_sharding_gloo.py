@@ -85,3 +85,36 @@ def test_two_rank_cost_based_slices(tmp_path):
     mp.spawn(_worker_cost, args=(2, port, str(tmp_path)), nprocs=2, join=True)
     a, b = np.load(tmp_path / "r0.npy"), np.load(tmp_path / "r1.npy")
     assert a[0] == 0 and a[0] + a[1] == b[0] and a[1] % 256 == 0 and b[1] % 256 == 0
+
+
+def test_regrouped_patch_costs_and_large_list_cuts():
+    """Cost model of regrouped layouts (1-cell patches packed into padded 16 x 16 blocks): every block of a level costs
+    the same whatever its fill, so the patches of a block share its cost; the slices of any world size partition
+    [0, N) at patch boundaries, and the prefix-sum path taken for long lists makes the cuts of the plain loop."""
+    from paper_2001_02765_b200 import sharding
+    from paper_2001_02765_b200.sharding import regrouped_patch_costs
+    from workloads import paper_ilr_layout
+    lay = paper_ilr_layout(64, 3)
+    costs = regrouped_patch_costs(lay.patches, lay.P)
+    key = (lay.patches[:, 0].astype(np.int64) << 40) | ((lay.patches[:, 2] >> 4).astype(np.int64) << 20) | (lay.patches[:, 1] >> 4)
+    n_blocks = [len(np.unique(key[lay.patches[:, 0] == l])) for l in range(lay.n_levels)]
+    for l in range(lay.n_levels):                                  # summed over a level: blocks of the level x all blocks
+        assert np.isclose(costs[lay.patches[:, 0] == l].sum(), n_blocks[l] * sum(n_blocks))
+    for world in (1, 2, 3, 8):
+        cuts = [shard_range_by_cost(costs, lay.P * lay.P, r, world) for r in range(world)]
+        assert cuts[0][0] == 0 and sum(c for _, c in cuts) == lay.n_cells
+        assert all(cuts[r][0] + cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))
+        share = [costs[f:f + c].sum() for f, c in cuts]
+        assert max(share) - min(share) <= 2.0 * costs.max() + 1e-9 # as even as whole patches allow
+    big = np.tile(costs, 100000 // len(costs) + 2)                 # > 100,000 entries: the numpy path
+    for world in (2, 5):
+        fast = [shard_range_by_cost(big, 1, r, world) for r in range(world)]
+        slow = [shard_range_by_cost(list(big[:90000]), 1, r, world) for r in range(world)]
+        ref = [sharding.shard_range_by_cost(big[:90000], 1, r, world) for r in range(world)]
+        assert slow == ref
+        total, acc, p, want_cuts = float(big.sum()), 0.0, 0, [0]
+        for r in range(1, world):                                  # the plain loop, restated
+            while p < len(big) and acc + 0.5 * big[p] <= total * r / world:
+                acc += big[p]; p += 1
+            want_cuts.append(p)
+        assert [f for f, _ in fast] == want_cuts
